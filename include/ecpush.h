@@ -1,0 +1,130 @@
+/*
+ * ecpush.h -- C ABI of libecpush: the particle hot path of the energy-conserving semi-implicit
+ * PIC scheme ECsim (arxiv 2603.16624; citations are PAPER.md lines) on one NVIDIA B200 (sm_100a).
+ *
+ * Per species the path is:
+ *   gather  E^{n+theta}, B^n at the particle with linear (CIC) weights W_pN        (L49, L88, L131-L133)
+ *   beta_p = q_p dt / (2 m_p);  alpha_p = (I - beta I x B_p + beta^2 B_p B_p)/(1+(beta B_p)^2)   (Eq. 2)
+ *   vbar = alpha_p (v^n + beta_p E_p);  v^{n+1} = 2 vbar - v^n;  x += dt v^{n+1}, periodic wrap (Eq. 6-8)
+ *   rho_N  += q_p W_pN / V_N                                                          (L147)
+ *   Jhat_N += q_p W_pN (alpha_p v_p^n) / V_N                                          (Eq. 1)
+ *   M^{ij}_{NN'} += beta_p q_p alpha_p^{ij} W_pN W_pN' / V_N,  27 neighbours N' of N  (Eq. 3)
+ * with the deposits taken at the pre-push position and velocity (L49).
+ *
+ * Conventions
+ *   - Every function returns 0 (ECSIM_OK) or a negative ecsim_status; nothing throws, aborts or exits.
+ *   - "device" pointers are CUDA device memory of the context's device, allocated and owned by the
+ *     caller (PyTorch in the harness).  The library BORROWS them: particle arrays from
+ *     ecsim_load_particles until the next load of that species / ecsim_destroy; the workspace from
+ *     ecsim_set_workspace until replaced / destroy; field and moment arrays only during the call
+ *     (stream-ordered).  The library owns only its small host context and a few CUDA events.
+ *   - All work is enqueued on the context's stream; no call synchronises with the host unless
+ *     its comment says so.
+ *   - Grid: periodic, nx*ny*nz cells = nodes; node n = (i*ny + j)*nz + k (z fastest, L127).
+ *     A particle's cell is the node id of its lower corner N- = floor(x/dx) per axis (L131).
+ *   - Fields:   F[c*nodes + n], c = 0,1,2 (x,y,z), double.
+ *   - Moments:  rho[n];  Jhat[c*nodes + n];  M[((n*27 + o)*3 + i)*3 + j] with neighbour slot
+ *     o = (di+1)*9 + (dj+1)*3 + (dk+1), di,dj,dk in {-1,0,1} (self = 13, mirror slot = 26-o),
+ *     i = row, j = column of alpha^{ij}.  All 27 slots are produced (L73 stores 14 by symmetry).
+ *   - Particles: structure of arrays of double: x,y,z (position, in [0,L)), u,v,w (velocity),
+ *     q (charge of the macro-particle); q_p/m_p is one number per species.
+ */
+#ifndef ECPUSH_H
+#define ECPUSH_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ecsim_ctx ecsim_ctx;
+
+enum ecsim_status {
+    ECSIM_OK = 0,
+    ECSIM_ERR_INVALID_ARG = -1, /* null pointer, n < 0, dims < 2, spacing <= 0, dt <= 0, theta outside [0.5,1], bad species */
+    ECSIM_ERR_NOT_LOADED = -2,  /* species has no particles loaded */
+    ECSIM_ERR_WORKSPACE = -3,   /* workspace missing or smaller than ecsim_workspace_bytes() */
+    ECSIM_ERR_CUDA = -4,        /* a CUDA call failed; text via ecsim_last_error() */
+    ECSIM_ERR_NOMEM = -5        /* host allocation failed */
+};
+
+/* Kernel variants of ecsim_push_and_moments (ecsim_set_variant). */
+enum ecsim_variant {
+    ECSIM_VARIANT_ATOMIC = 0, /* the paper's design (L143): one thread per particle, one global atomic per
+                                 scalar contribution; correct for any particle order                    */
+    ECSIM_VARIANT_FUSED = 1   /* default: cell-sorted tiles, per-cell register accumulators (27 weight-product
+                                 classes x 9 + Jhat + rho), one flush per cell; strays take the atomic path */
+};
+
+/* Create a context for a periodic grid of nx*ny*nz cells (each >= 2) with spacing dx,dy,dz (> 0).
+ * cuda_stream is a cudaStream_t (NULL = legacy default stream) on the CURRENT device.  *ctx receives the context. */
+int ecsim_init_grid(ecsim_ctx **ctx, int nx, int ny, int nz, double dx, double dy, double dz,
+                    int n_species, void *cuda_stream);
+
+/* Scratch bytes needed for species holding at most n_particles_max particles each:
+ * sort keys, permutation, per-cell counters/offsets and one spare particle SoA for out-of-place sorting. */
+size_t ecsim_workspace_bytes(const ecsim_ctx *ctx, int64_t n_particles_max);
+
+/* Lend device scratch (256-byte aligned).  Host-only call. */
+int ecsim_set_workspace(ecsim_ctx *ctx, void *dev_ptr, size_t bytes);
+
+/* Register the device SoA of one species (n >= 0 particles, q_over_m = q_p/m_p).  x..w are updated in
+ * place by push and by sort; q is permuted by sort.  `sorted` != 0 declares the arrays cell-sorted
+ * (a performance hint only: particles found outside their cell's segment are still deposited correctly). */
+int ecsim_load_particles(ecsim_ctx *ctx, int species, int64_t n, double q_over_m,
+                         double *x, double *y, double *z, double *u, double *v, double *w, double *q,
+                         int sorted);
+
+/* Counting sort of the species by cell id (L149: the sort the paper could not realise with OpenACC).
+ * On return (stream-ordered) the caller's arrays hold the particles grouped by cell, cells ascending;
+ * order within a cell is unspecified.  cell_count_out: device int32[cells] per-cell counts, or NULL.
+ * perm_out: device uint32[n], perm_out[new] = old index, or NULL. */
+int ecsim_sort_particles(ecsim_ctx *ctx, int species, int32_t *cell_count_out, uint32_t *perm_out);
+
+/* Cell id of every particle as stored now: device int32[n].  (Parity of the integer binning.) */
+int ecsim_cell_index(ecsim_ctx *ctx, int species, int32_t *cell_out);
+
+/* One hot-path step for one species: gather, alpha, push, deposit (header of this file).
+ *   E_theta, B : device [3][nodes], E^{n+theta} and B^n at nodes
+ *   dt > 0; theta in [0.5, 1] is validated and stored, no formula of this path uses it (L84)
+ *   rho [nodes], Jhat [3][nodes], M [nodes][27][3][3]: device outputs; any may be NULL (skipped)
+ *   accumulate : 0 = outputs are zeroed first; 1 = contributions are added (sum over species, L59 L84)
+ * With variant FUSED an unsorted species is sorted first (same effect as ecsim_sort_particles).
+ * After the call the species is marked unsorted (particles moved). */
+int ecsim_push_and_moments(ecsim_ctx *ctx, int species, const double *E_theta, const double *B,
+                           double dt, double theta, double *rho, double *Jhat, double *M, int accumulate);
+
+/* Same step with HOST buffers: copies particles and fields to device staging (carved from the
+ * workspace, which must be ecsim_host_step_workspace_bytes() large), runs the step, copies particles
+ * and moments back, and synchronises the stream.  Host arrays: x..w in/out [n], q in [n], E/B in,
+ * rho/Jhat/M out (accumulate: M etc. are read first).  Pinned host memory makes the copies asynchronous. */
+size_t ecsim_host_step_workspace_bytes(const ecsim_ctx *ctx, int64_t n_particles);
+int ecsim_push_and_moments_host(ecsim_ctx *ctx, int64_t n, double q_over_m, int sorted,
+                                double *x, double *y, double *z, double *u, double *v, double *w,
+                                const double *q, const double *E_theta, const double *B,
+                                double dt, double theta, double *rho, double *Jhat, double *M, int accumulate);
+
+/* Select the kernel variant (default ECSIM_VARIANT_FUSED). */
+int ecsim_set_variant(ecsim_ctx *ctx, int variant);
+
+/* Instrumentation.  ecsim_enable_timing(1) records CUDA events around the deposit/push kernel of every
+ * ecsim_push_and_moments call; ecsim_kernel_ms() SYNCHRONISES on the last pair and returns its time.
+ * ecsim_launch_count() = kernels + memsets this context has enqueued so far;
+ * ecsim_stray_count() = particles the last FUSED step found outside their segment (device->host sync). */
+int ecsim_enable_timing(ecsim_ctx *ctx, int on);
+int ecsim_kernel_ms(ecsim_ctx *ctx, float *ms_out);
+int64_t ecsim_launch_count(const ecsim_ctx *ctx);
+int64_t ecsim_stray_count(ecsim_ctx *ctx);
+
+int ecsim_destroy(ecsim_ctx *ctx);
+
+/* Static text for a status; ecsim_last_error: text of the last CUDA failure in this process. */
+const char *ecsim_strerror(int status);
+const char *ecsim_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ECPUSH_H */
