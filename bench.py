@@ -1,0 +1,401 @@
+#!/usr/bin/env python
+"""bench.py -- particles pushed + mass-matrix-deposited per second (FP64) on B200, libecpush.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl reference]
+
+A "step" is one pass of the whole hot path (gather, alpha, push, deposit of
+rho/Jhat/M, per-cell pre-reduction and flush) over every particle of every species of the workload,
+through the C ABI (ecsim_push_and_moments_all), starting from the cell-sorted state.  Default
+workload: BASELINE.json configs[2] (128^3 cells, 2 species x 64 ppc = 268,435,456 particles), the
+configuration the metric is quoted on.  Protocol: inputs
+resident in HBM; each step timed with CUDA events on the library's stream; the particle state is
+restored from a pristine device copy between steps, outside the timed region; the working set
+(15 GB of particles, 4 GB of M) is far larger than the 126 MB L2, so no explicit flush is needed.
+
+One JSON line on stdout (rank 0).  `--impl reference` times the CPU oracle (oracle/, as it
+stands, single thread) on a bounded sample of the same workload instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+for _p in (ROOT, os.path.join(ROOT, "tests")):
+    if _p not in sys.path:
+        sys.path.insert(0, _p)
+
+METRIC = "particles pushed+mass-matrix-deposited per sec (FP64); % of B200 roofline"
+UNIT = "particles/s"
+# algorithmic FP64 work per particle in the minimum (27-class) formulation and
+# algorithmic HBM bytes per particle at 128 particles per node.
+FLOP_PER_PARTICLE = 813.0
+BYTES_PER_PARTICLE_CFG2 = 119.8
+# FP64 vector peak derived from unit counts and clocks: 148 SM x 64 FMA/clk x 2 flop x 1.965 GHz
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+NORTH_STAR_ROOFLINE_PPS = min(8.0e12 / BYTES_PER_PARTICLE_CFG2, FP64_PEAK_TFLOPS * 1e12 / FLOP_PER_PARTICLE)
+# dram__bytes_read.sum + dram__bytes_write.sum of k_fused_push_moments per launch, from the ncu
+# --set full capture summarised in profiles/ (None until a capture of this workload exists)
+FUSED_DRAM_TRAFFIC_BYTES = None
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="libecpush", choices=["libecpush", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (default 2, the headline)")
+    ap.add_argument("--scale", default=None, help="nx,ny,nz override of the grid (tests / quick runs)")
+    ap.add_argument("--variant", default="fused", choices=["fused", "atomic"])
+    ap.add_argument("--fused-warps", type=int, default=0)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--cpu-sample-planes", type=int, default=2, help="x-planes of cells the oracle sample covers")
+    return ap.parse_args()
+
+
+# ------------------------------------------------------------------------------------------------
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+def max_over_ranks(values, world, backend_device="cuda"):
+    """Element-wise max of a list of floats over all ranks (torch.distributed); identity at world 1."""
+    if world == 1:
+        return list(values)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(values, dtype=torch.float64, device=backend_device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.cpu()]
+
+
+def sum_over_ranks(value, world, backend_device="cuda"):
+    if world == 1:
+        return value
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=backend_device)
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.cpu()[0])
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+
+    QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+             "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu = gpu_index
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.QUERY}", "--format=csv,noheader,nounits", "-lms", "100",
+                 "-i", str(self.gpu)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except Exception:
+            self.proc.kill()
+            out = ""
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); smax.append(float(f[2])); power.append(float(f[3]))
+            except ValueError:
+                continue
+            for name, val in zip(names, f[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        # under load = samples drawing more than half of the maximum power seen
+        pmax = max(power)
+        loaded = [c for c, p in zip(sm, power) if p >= 0.5 * pmax] or sm
+        return {"sm_mhz": statistics.median(loaded), "sm_max_mhz": max(smax), "reasons": sorted(reasons),
+                "power_w_max": pmax, "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------------
+def load_config(args):
+    import workloads as wl
+    scale = tuple(int(v) for v in args.scale.split(",")) if args.scale else None
+    return wl.config(args.config, scale)
+
+
+def workload_name(cfg):
+    n = None
+    return f"BASELINE.json configs[{cfg.idx}] {cfg.name}: {cfg.nx}x{cfg.ny}x{cfg.nz} cells, {len(cfg.species)} species"
+
+
+def oracle_sample(cfg, planes, with_e2e_keys=True):
+    """Time the CPU oracle (as it stands: plain C, one thread) on the particles of the first `planes`
+    x-planes of cells of the workload, on the full-size grid.  Returns (particles/s, n, seconds, cores)."""
+    import numpy as np
+    import oracle
+    import workloads as wl
+    from util import grid_of, to_numpy
+    planes = max(1, min(planes, cfg.nx))
+    cells = list(range(planes * cfg.ny * cfg.nz))
+    E, B = wl.gen_fields(cfg)
+    En, Bn = E.numpy(), B.numpy()
+    parts = [to_numpy(wl.gen_species(cfg, s, cells=cells)) for s in range(len(cfg.species))]
+    n = sum(p["x"].shape[0] for p in parts)
+    mom = oracle.Moments(cfg.nodes, with_abs=False)      # calloc-backed: only touched pages are committed
+    oracle.lib()
+    t0 = time.perf_counter()
+    for s, sp in enumerate(cfg.species):
+        oracle.step(grid_of(cfg), sp.qom, cfg.dt, parts[s], En, Bn, mom)
+    dt = time.perf_counter() - t0
+    return n / dt, n, dt, 1
+
+
+def run_reference(args):
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return
+    cfg = load_config(args)
+    for _ in range(max(0, args.warmup)):
+        oracle_sample(cfg, 1)
+    rates, secs, n = [], [], 0
+    for _ in range(max(1, args.steps)):
+        r, n, dt, cores = oracle_sample(cfg, args.cpu_sample_planes)
+        rates.append(r); secs.append(dt)
+    value = n * len(secs) / sum(secs)
+    sample = (f"particles of the first {min(args.cpu_sample_planes, cfg.nx)} x-planes of cells "
+              f"({n} particles, all species) on the full {cfg.nx}x{cfg.ny}x{cfg.nz} grid, one oracle step per bench step")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sum(secs) / len(secs),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "note": "CPU oracle (oracle/ecsim_oracle.c, gcc -O2 -ffp-contract=off), "
+                   "host cores of this box; ms_per_step is per sample, not per full workload"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------
+def run_product(args):
+    import torch
+    import paper_2603_16624_b200 as pk
+    import workloads as wl
+    from util import PKEYS, grid_of
+
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; libecpush has no CPU fallback")
+    torch.cuda.set_device(local % torch.cuda.device_count())
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl")
+    cfg = load_config(args)
+    dev = torch.device("cuda")
+    nsp = len(cfg.species)
+
+    # ---- synthetic inputs, resident in HBM (every rank: an independent replica of the workload) ----
+    E, B = wl.gen_fields(cfg, device=dev)
+    pristine = []
+    for s in range(nsp):
+        p = wl.gen_species(cfg, s, device=dev)
+        pristine.append({k: p[k].contiguous() for k in PKEYS})
+        del p
+    torch.cuda.empty_cache()
+    n_s = [int(p["x"].numel()) for p in pristine]
+    n_total = sum(n_s)
+    work = [{k: torch.empty_like(p[k]) for k in PKEYS} for p in pristine]
+    for s in range(nsp):
+        work[s]["q"].copy_(pristine[s]["q"])
+
+    ctx = pk.Ecsim(*grid_of(cfg), nsp)
+    ctx.set_workspace(max(n_s))
+    ctx.set_variant(pk.VARIANT_FUSED if args.variant == "fused" else pk.VARIANT_ATOMIC)
+    if args.fused_warps:
+        ctx.set_fused_warps(args.fused_warps)
+    ctx.enable_timing(True)
+    rho = torch.empty(nsp, cfg.nodes, dtype=torch.float64, device=dev)
+    J = torch.empty(nsp, 3, cfg.nodes, dtype=torch.float64, device=dev)
+    M = torch.empty(cfg.nodes, 27, 3, 3, dtype=torch.float64, device=dev)
+    sorted_input = not cfg.shuffled
+
+    def restore():
+        for s in range(nsp):
+            for k in ("x", "y", "z", "u", "v", "w") + (("q",) if cfg.shuffled else ()):
+                work[s][k].copy_(pristine[s][k])
+            ctx.load_particles(s, cfg.species[s].qom, work[s], sorted=sorted_input)
+            if sorted_input:
+                ctx.build_segments(s)        # set-up of the sorted state, not part of the step
+
+    def one_step():
+        ctx.push_and_moments_all(E, B, cfg.dt, cfg.theta, rho, J, M, accumulate=pk.ACC_NONE)
+
+    fp64_probe, _ = ctx.probe_fp64(4096)
+
+    for _ in range(max(3, args.warmup)):
+        restore()
+        one_step()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+
+    sampler = ClockSampler(torch.cuda.current_device())
+    sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    kernel_ms = []
+    launches0 = ctx.launch_count()
+    launches_step = 0
+    torch.cuda.synchronize()
+    for i in range(args.steps):
+        restore()
+        torch.cuda.synchronize()
+        l0 = ctx.launch_count()
+        ev[i][0].record()
+        one_step()
+        ev[i][1].record()
+        launches_step += ctx.launch_count() - l0
+        torch.cuda.synchronize()
+        kernel_ms.append(ctx.kernel_ms())
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    clocks = sampler.stop()
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = max_over_ranks([sum(step_ms)], world)[0]
+    ms_per_step = total_ms / args.steps
+    value = world * n_total * args.steps / (total_ms * 1e-3)
+    k_ms = sum(kernel_ms) / len(kernel_ms)
+    achieved_tflops = FLOP_PER_PARTICLE * n_total / (k_ms * 1e-3) / 1e12
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {
+            "workload": workload_name(cfg), "particles": n_total, "variant": args.variant,
+            "multi_gpu": "replicas only (north_star: single GPU; each rank runs the whole workload)",
+            "l2": "inputs (>= 15 GB at configs[2]) exceed the 126 MB L2; no explicit flush" if n_total * 56 > 2e9
+                  else "working set may fit L2 (small config): not a headline number",
+            "timing": "per-step CUDA events; particle state restored from a pristine device copy between steps, "
+                      "outside the timed region; outputs written inside",
+        },
+        "roofline": {
+            "bound": "alu", "kernel": "k_fused_push_moments" if args.variant == "fused" else "k_push_moments_atomic",
+            "achieved": achieved_tflops, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved_tflops / FP64_PEAK_TFLOPS,
+            "traffic": FUSED_DRAM_TRAFFIC_BYTES if (args.variant == "fused" and cfg.idx == 2 and not args.scale) else None,
+            "peak_source": "derived: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md); fp64_probe_tflops is the DFMA "
+                           "micro-benchmark measured in this run",
+            "fp64_probe_tflops": fp64_probe, "kernel_ms": k_ms, "flop_per_particle": FLOP_PER_PARTICLE,
+            "kernel_share_of_step": k_ms / ms_per_step,
+        },
+        "north_star_roofline": {"particles_per_s": NORTH_STAR_ROOFLINE_PPS, "frac": value / world / NORTH_STAR_ROOFLINE_PPS,
+                                "definition": "slower of 119.8 B/particle at 8 TB/s and 813 flop/particle at 37.2 TFLOP/s"},
+        "gpu_launches": launches_step,
+        "clocks": clocks,
+    }
+
+    # ---- end to end through the host-buffer entry point (rank-local, pinned host memory) ----
+    if not args.no_e2e:
+        line["e2e"] = run_e2e(args, cfg, ctx, pristine, E, B, world)
+    else:
+        line["e2e"] = None
+    ctx.close()
+    del work, pristine, M
+    torch.cuda.empty_cache()
+
+    if rank == 0 and not args.no_cpu_baseline and world == 1:
+        v, n, dt, cores = oracle_sample(cfg, args.cpu_sample_planes)
+        line["cpu_baseline"] = {
+            "value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"particles of the first {min(args.cpu_sample_planes, cfg.nx)} x-planes of cells ({n} particles, "
+                      f"all species) on the full grid; {dt:.1f} s of CPU work"}
+    else:
+        line["cpu_baseline"] = None
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def run_e2e(args, cfg, ctx_unused, pristine, E, B, world):
+    """Same metric through ecsim_push_and_moments_host: pinned host buffers in, host buffers out, the
+    host<->device copies inside the timed region."""
+    import torch
+    import paper_2603_16624_b200 as pk
+    from util import PKEYS, grid_of
+    nsp = len(cfg.species)
+    n_s = [int(p["x"].numel()) for p in pristine]
+    host = [{k: torch.empty(n_s[s], dtype=torch.float64).pin_memory() for k in PKEYS} for s in range(nsp)]
+    Eh, Bh = E.cpu().pin_memory(), B.cpu().pin_memory()
+    rho = torch.empty(nsp, cfg.nodes, dtype=torch.float64).pin_memory()
+    J = torch.empty(nsp, 3, cfg.nodes, dtype=torch.float64).pin_memory()
+    M = torch.empty(cfg.nodes, 27, 3, 3, dtype=torch.float64).pin_memory()
+    ctx = pk.Ecsim(*grid_of(cfg), 1)
+    ctx.set_workspace(max(n_s), host_step=True)
+    if args.variant == "atomic":
+        ctx.set_variant(pk.VARIANT_ATOMIC)
+
+    def refill():
+        for s in range(nsp):
+            for k in PKEYS:
+                host[s][k].copy_(pristine[s][k])
+        torch.cuda.synchronize()
+
+    def step():
+        for s in range(nsp):
+            ctx.push_and_moments_host(cfg.species[s].qom, not cfg.shuffled, host[s], Eh, Bh, cfg.dt, cfg.theta,
+                                      rho[s], J[s], M, accumulate=(pk.ACC_M_ONLY if s > 0 else pk.ACC_NONE))
+
+    refill(); step()                                   # warm-up
+    times = []
+    for _ in range(max(1, args.e2e_steps)):
+        refill()
+        t0 = time.perf_counter()
+        step()                                         # each host call ends with a stream synchronise
+        times.append(time.perf_counter() - t0)
+    ctx.close()
+    t = max_over_ranks([sum(times)], world)[0]
+    n_total = sum(n_s)
+    nodes = cfg.nodes
+    h2d = sum(7 * 8 * n for n in n_s) + nsp * 6 * 8 * nodes + (nsp - 1) * 243 * 8 * nodes
+    d2h = sum(6 * 8 * n for n in n_s) + nsp * (243 + 4) * 8 * nodes
+    return {"value": world * n_total * len(times) / t, "unit": UNIT, "h2d_bytes_per_step": h2d,
+            "d2h_bytes_per_step": d2h, "steps": len(times),
+            "api": "ecsim_push_and_moments_host, one call per species, pinned host memory, copies inside the timed region"}
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_product(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -50,12 +50,21 @@ enum ecsim_status {
     ECSIM_ERR_NOMEM = -5        /* host allocation failed */
 };
 
+/* `accumulate` argument of the push_and_moments calls. */
+enum ecsim_accumulate {
+    ECSIM_ACC_NONE = 0,  /* every output is overwritten */
+    ECSIM_ACC_ALL = 1,   /* contributions are added to rho, Jhat and M (sum over species, L84) */
+    ECSIM_ACC_M_ONLY = 2 /* added to M (mass matrices are summed over species, L59); rho and Jhat of this
+                            species are overwritten (Jhat is kept per species, L129) */
+};
+
 /* Kernel variants of ecsim_push_and_moments (ecsim_set_variant). */
 enum ecsim_variant {
     ECSIM_VARIANT_ATOMIC = 0, /* the paper's design (L143): one thread per particle, one global atomic per
                                  scalar contribution; correct for any particle order                    */
-    ECSIM_VARIANT_FUSED = 1   /* default: cell-sorted tiles, per-cell register accumulators (27 weight-product
-                                 classes x 9 + Jhat + rho), one flush per cell; strays take the atomic path */
+    ECSIM_VARIANT_FUSED = 1   /* default: cell-sorted particles, one warp per cell, per-cell register accumulators
+                                 (27 weight-product classes x 9 + Jhat + rho) written once per cell with plain
+                                 stores and expanded to the node arrays; strays take the atomic path */
 };
 
 /* Create a context for a periodic grid of nx*ny*nz cells (each >= 2) with spacing dx,dy,dz (> 0).
@@ -63,8 +72,9 @@ enum ecsim_variant {
 int ecsim_init_grid(ecsim_ctx **ctx, int nx, int ny, int nz, double dx, double dy, double dz,
                     int n_species, void *cuda_stream);
 
-/* Scratch bytes needed for species holding at most n_particles_max particles each:
- * sort keys, permutation, per-cell counters/offsets and one spare particle SoA for out-of-place sorting. */
+/* Scratch bytes needed for species holding at most n_particles_max particles each: per-species cell segment
+ * tables, sort keys / ranks / permutation, one spare array for the out-of-place permutation, stray lists,
+ * and the per-cell accumulator arrays AM[cells][27][9], AJ[n_species][cells][8][4] of the fused kernel. */
 size_t ecsim_workspace_bytes(const ecsim_ctx *ctx, int64_t n_particles_max);
 
 /* Lend device scratch (256-byte aligned).  Host-only call. */
@@ -72,7 +82,8 @@ int ecsim_set_workspace(ecsim_ctx *ctx, void *dev_ptr, size_t bytes);
 
 /* Register the device SoA of one species (n >= 0 particles, q_over_m = q_p/m_p).  x..w are updated in
  * place by push and by sort; q is permuted by sort.  `sorted` != 0 declares the arrays cell-sorted
- * (a performance hint only: particles found outside their cell's segment are still deposited correctly). */
+ * (a performance hint only: particles found outside their cell's segment are still deposited correctly).
+ * Host-only call: no device work is enqueued. */
 int ecsim_load_particles(ecsim_ctx *ctx, int species, int64_t n, double q_over_m,
                          double *x, double *y, double *z, double *u, double *v, double *w, double *q,
                          int sorted);
@@ -83,6 +94,11 @@ int ecsim_load_particles(ecsim_ctx *ctx, int species, int64_t n, double q_over_m
  * perm_out: device uint32[n], perm_out[new] = old index, or NULL. */
 int ecsim_sort_particles(ecsim_ctx *ctx, int species, int32_t *cell_count_out, uint32_t *perm_out);
 
+/* Build the per-cell segment table (start[cells+1]) of a species whose arrays are ALREADY cell-sorted
+ * (histogram + exclusive scan, no particle moves).  ecsim_push_and_moments does this by itself for a
+ * species loaded with sorted != 0; calling it first keeps that set-up out of a timed step. */
+int ecsim_build_segments(ecsim_ctx *ctx, int species);
+
 /* Cell id of every particle as stored now: device int32[n].  (Parity of the integer binning.) */
 int ecsim_cell_index(ecsim_ctx *ctx, int species, int32_t *cell_out);
 
@@ -90,16 +106,25 @@ int ecsim_cell_index(ecsim_ctx *ctx, int species, int32_t *cell_out);
  *   E_theta, B : device [3][nodes], E^{n+theta} and B^n at nodes
  *   dt > 0; theta in [0.5, 1] is validated and stored, no formula of this path uses it (L84)
  *   rho [nodes], Jhat [3][nodes], M [nodes][27][3][3]: device outputs; any may be NULL (skipped)
- *   accumulate : 0 = outputs are zeroed first; 1 = contributions are added (sum over species, L59 L84)
- * With variant FUSED an unsorted species is sorted first (same effect as ecsim_sort_particles).
- * After the call the species is marked unsorted (particles moved). */
+ *   accumulate : enum ecsim_accumulate
+ * With variant FUSED an unsorted species is sorted first (same effect as ecsim_sort_particles).  After the
+ * call the species keeps its segment table; the kernel counts the particles that left their cell, and the
+ * next call re-sorts first when that count exceeds ecsim_set_resort_fraction() * n (default 1 %), otherwise
+ * the leavers are handled as strays by the atomic path.  (The count is read through pinned memory: the next
+ * call waits for this call's kernels to finish before it decides.) */
 int ecsim_push_and_moments(ecsim_ctx *ctx, int species, const double *E_theta, const double *B,
                            double dt, double theta, double *rho, double *Jhat, double *M, int accumulate);
+
+/* The same step for ALL species of the context in one pass (the mass matrices are summed over species, L59;
+ * Jhat is kept per species, L129): each cell's particles of every species go through the same per-cell
+ * accumulators, so M is flushed once.  rho [n_species][nodes], Jhat [n_species][3][nodes], M as above. */
+int ecsim_push_and_moments_all(ecsim_ctx *ctx, const double *E_theta, const double *B, double dt, double theta,
+                               double *rho, double *Jhat, double *M, int accumulate);
 
 /* Same step with HOST buffers: copies particles and fields to device staging (carved from the
  * workspace, which must be ecsim_host_step_workspace_bytes() large), runs the step, copies particles
  * and moments back, and synchronises the stream.  Host arrays: x..w in/out [n], q in [n], E/B in,
- * rho/Jhat/M out (accumulate: M etc. are read first).  Pinned host memory makes the copies asynchronous. */
+ * rho/Jhat/M out (with accumulate != 0 the accumulated arrays are copied in first).  Pinned host memory makes the copies asynchronous. */
 size_t ecsim_host_step_workspace_bytes(const ecsim_ctx *ctx, int64_t n_particles);
 int ecsim_push_and_moments_host(ecsim_ctx *ctx, int64_t n, double q_over_m, int sorted,
                                 double *x, double *y, double *z, double *u, double *v, double *w,
@@ -109,14 +134,24 @@ int ecsim_push_and_moments_host(ecsim_ctx *ctx, int64_t n, double q_over_m, int 
 /* Select the kernel variant (default ECSIM_VARIANT_FUSED). */
 int ecsim_set_variant(ecsim_ctx *ctx, int variant);
 
+/* Tuning knobs: fraction of a species that may sit outside its cell segment before the next step re-sorts
+ * (default 0.01); warps per CTA of the fused kernel (8, 12 or 16; default 12). */
+int ecsim_set_resort_fraction(ecsim_ctx *ctx, double fraction);
+int ecsim_set_fused_warps(ecsim_ctx *ctx, int warps);
+
 /* Instrumentation.  ecsim_enable_timing(1) records CUDA events around the deposit/push kernel of every
  * ecsim_push_and_moments call; ecsim_kernel_ms() SYNCHRONISES on the last pair and returns its time.
  * ecsim_launch_count() = kernels + memsets this context has enqueued so far;
- * ecsim_stray_count() = particles the last FUSED step found outside their segment (device->host sync). */
+ * ecsim_stray_count() = particles the last FUSED step found outside their segment (synchronises the stream). */
 int ecsim_enable_timing(ecsim_ctx *ctx, int on);
 int ecsim_kernel_ms(ecsim_ctx *ctx, float *ms_out);
 int64_t ecsim_launch_count(const ecsim_ctx *ctx);
 int64_t ecsim_stray_count(ecsim_ctx *ctx);
+int64_t ecsim_resort_count(const ecsim_ctx *ctx); /* re-sorts ecsim_push_and_moments triggered so far */
+
+/* FP64 FMA throughput of the device (dependent-chain DFMA kernel, `iters` x 128 FMAs per thread), the
+ * denominator of the ALU roofline.  Synchronises.  tflops_out: 2 flops per FMA; ms_out may be NULL. */
+int ecsim_probe_fp64(ecsim_ctx *ctx, int iters, double *tflops_out, float *ms_out);
 
 int ecsim_destroy(ecsim_ctx *ctx);
 

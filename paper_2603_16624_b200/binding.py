@@ -1,0 +1,239 @@
+"""ctypes binding of libecpush.so (include/ecpush.h).  Argument marshalling only.
+
+`lib()` returns the loaded library with typed prototypes named exactly as in the header.
+`Ecsim` is a small convenience wrapper that owns an `ecsim_ctx*`, lets PyTorch allocate the
+workspace, and forwards torch CUDA tensors as raw device pointers.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import re
+from typing import Optional, Sequence
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+ROOT = os.path.dirname(HERE)
+HEADER = os.path.join(ROOT, "include", "ecpush.h")
+
+VARIANT_ATOMIC = 0
+VARIANT_FUSED = 1
+ACC_NONE = 0
+ACC_ALL = 1
+ACC_M_ONLY = 2
+
+_c = ctypes
+_P = _c.c_void_p
+_lib = None
+
+
+class EcsimError(RuntimeError):
+    pass
+
+
+def lib_path() -> str:
+    return os.path.join(HERE, "libecpush.so")
+
+
+def declared_symbols() -> list:
+    """Names of every function include/ecpush.h declares (used by the ABI test)."""
+    text = open(HEADER).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(ecsim_[a-z0-9_]+)\s*\(", text)))
+
+
+_PROTOS = {
+    "ecsim_init_grid": (_c.c_int, [_c.POINTER(_P), _c.c_int, _c.c_int, _c.c_int, _c.c_double, _c.c_double,
+                                   _c.c_double, _c.c_int, _P]),
+    "ecsim_workspace_bytes": (_c.c_size_t, [_P, _c.c_int64]),
+    "ecsim_set_workspace": (_c.c_int, [_P, _P, _c.c_size_t]),
+    "ecsim_load_particles": (_c.c_int, [_P, _c.c_int, _c.c_int64, _c.c_double] + [_P] * 7 + [_c.c_int]),
+    "ecsim_sort_particles": (_c.c_int, [_P, _c.c_int, _P, _P]),
+    "ecsim_build_segments": (_c.c_int, [_P, _c.c_int]),
+    "ecsim_cell_index": (_c.c_int, [_P, _c.c_int, _P]),
+    "ecsim_push_and_moments": (_c.c_int, [_P, _c.c_int, _P, _P, _c.c_double, _c.c_double, _P, _P, _P, _c.c_int]),
+    "ecsim_push_and_moments_all": (_c.c_int, [_P, _P, _P, _c.c_double, _c.c_double, _P, _P, _P, _c.c_int]),
+    "ecsim_host_step_workspace_bytes": (_c.c_size_t, [_P, _c.c_int64]),
+    "ecsim_push_and_moments_host": (_c.c_int, [_P, _c.c_int64, _c.c_double, _c.c_int] + [_P] * 9 +
+                                    [_c.c_double, _c.c_double, _P, _P, _P, _c.c_int]),
+    "ecsim_set_variant": (_c.c_int, [_P, _c.c_int]),
+    "ecsim_set_resort_fraction": (_c.c_int, [_P, _c.c_double]),
+    "ecsim_set_fused_warps": (_c.c_int, [_P, _c.c_int]),
+    "ecsim_enable_timing": (_c.c_int, [_P, _c.c_int]),
+    "ecsim_kernel_ms": (_c.c_int, [_P, _c.POINTER(_c.c_float)]),
+    "ecsim_launch_count": (_c.c_int64, [_P]),
+    "ecsim_stray_count": (_c.c_int64, [_P]),
+    "ecsim_resort_count": (_c.c_int64, [_P]),
+    "ecsim_probe_fp64": (_c.c_int, [_P, _c.c_int, _c.POINTER(_c.c_double), _c.POINTER(_c.c_float)]),
+    "ecsim_destroy": (_c.c_int, [_P]),
+    "ecsim_strerror": (_c.c_char_p, [_c.c_int]),
+    "ecsim_last_error": (_c.c_char_p, []),
+}
+
+
+def lib():
+    """Load libecpush.so (built in-tree by paper_2603_16624_b200.build).  Fails loudly."""
+    global _lib
+    if _lib is None:
+        path = lib_path()
+        if not os.path.exists(path):
+            raise EcsimError(f"{path} is missing: build it with `python -m paper_2603_16624_b200.build` "
+                             "(there is no CPU fallback)")
+        L = _c.CDLL(path)
+        for name, (res, args) in _PROTOS.items():
+            fn = getattr(L, name)
+            fn.restype = res
+            fn.argtypes = args
+        _lib = L
+    return _lib
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        L = lib()
+        raise EcsimError(f"{what}: {L.ecsim_strerror(rc).decode()} [{rc}] {L.ecsim_last_error().decode()}")
+
+
+def _dptr(t, dtype=None):
+    """Raw device pointer of a contiguous CUDA tensor (or None)."""
+    if t is None:
+        return None
+    if not t.is_cuda or not t.is_contiguous():
+        raise EcsimError("expected a contiguous CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise EcsimError(f"expected dtype {dtype}, got {t.dtype}")
+    return _P(t.data_ptr())
+
+
+def _hptr(t, dtype=None):
+    if t is None:
+        return None
+    if t.is_cuda or not t.is_contiguous():
+        raise EcsimError("expected a contiguous host tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise EcsimError(f"expected dtype {dtype}, got {t.dtype}")
+    return _P(t.data_ptr())
+
+
+class Ecsim:
+    """One libecpush context on the current CUDA device and (by default) torch's current stream."""
+
+    def __init__(self, nx: int, ny: int, nz: int, dx: float, dy: float, dz: float, n_species: int,
+                 stream=None):
+        import torch
+        self.torch = torch
+        if not torch.cuda.is_available():
+            raise EcsimError("libecpush needs a CUDA device (no CPU fallback)")
+        self.L = lib()
+        self.grid = (nx, ny, nz, dx, dy, dz)
+        self.nodes = nx * ny * nz
+        self.n_species = n_species
+        self.stream = stream if stream is not None else torch.cuda.current_stream()
+        h = _P()
+        _check(self.L.ecsim_init_grid(_c.byref(h), nx, ny, nz, dx, dy, dz, n_species,
+                                      _P(self.stream.cuda_stream)), "ecsim_init_grid")
+        self.h = h
+        self._ws = None
+        self._keep = {}
+
+    # -- workspace -----------------------------------------------------------------------------
+    def workspace_bytes(self, n_max: int) -> int:
+        return int(self.L.ecsim_workspace_bytes(self.h, n_max))
+
+    def host_step_workspace_bytes(self, n: int) -> int:
+        return int(self.L.ecsim_host_step_workspace_bytes(self.h, n))
+
+    def set_workspace(self, n_max: int, host_step: bool = False):
+        """Let torch allocate the scratch and lend it to the library."""
+        nbytes = self.host_step_workspace_bytes(n_max) if host_step else self.workspace_bytes(n_max)
+        ws = self.torch.empty(nbytes + 256, dtype=self.torch.uint8, device="cuda")
+        off = (-ws.data_ptr()) % 256
+        self._ws = ws
+        _check(self.L.ecsim_set_workspace(self.h, _P(ws.data_ptr() + off), nbytes), "ecsim_set_workspace")
+        return nbytes
+
+    # -- particles -----------------------------------------------------------------------------
+    def load_particles(self, species: int, qom: float, part: dict, sorted: bool = False):
+        f64 = self.torch.float64
+        n = int(part["x"].numel())
+        ptrs = [_dptr(part[k], f64) for k in ("x", "y", "z", "u", "v", "w", "q")]
+        self._keep[species] = part
+        _check(self.L.ecsim_load_particles(self.h, species, n, qom, *ptrs, 1 if sorted else 0),
+               "ecsim_load_particles")
+
+    def sort_particles(self, species: int, cell_count_out=None, perm_out=None):
+        _check(self.L.ecsim_sort_particles(self.h, species, _dptr(cell_count_out, self.torch.int32),
+                                           _dptr(perm_out)), "ecsim_sort_particles")
+
+    def build_segments(self, species: int):
+        _check(self.L.ecsim_build_segments(self.h, species), "ecsim_build_segments")
+
+    def cell_index(self, species: int, cell_out):
+        _check(self.L.ecsim_cell_index(self.h, species, _dptr(cell_out, self.torch.int32)), "ecsim_cell_index")
+
+    # -- the hot path --------------------------------------------------------------------------
+    def push_and_moments(self, species: int, E, B, dt: float, theta: float, rho, Jhat, M, accumulate: int = 0):
+        f64 = self.torch.float64
+        _check(self.L.ecsim_push_and_moments(self.h, species, _dptr(E, f64), _dptr(B, f64), dt, theta,
+                                             _dptr(rho, f64), _dptr(Jhat, f64), _dptr(M, f64),
+                                             int(accumulate)), "ecsim_push_and_moments")
+
+    def push_and_moments_all(self, E, B, dt: float, theta: float, rho, Jhat, M, accumulate: int = 0):
+        f64 = self.torch.float64
+        _check(self.L.ecsim_push_and_moments_all(self.h, _dptr(E, f64), _dptr(B, f64), dt, theta,
+                                                 _dptr(rho, f64), _dptr(Jhat, f64), _dptr(M, f64),
+                                                 int(accumulate)), "ecsim_push_and_moments_all")
+
+    def push_and_moments_host(self, qom: float, sorted: bool, part: dict, E, B, dt: float, theta: float,
+                              rho, Jhat, M, accumulate: int = 0):
+        f64 = self.torch.float64
+        n = int(part["x"].numel())
+        ptrs = [_hptr(part[k], f64) for k in ("x", "y", "z", "u", "v", "w", "q")]
+        _check(self.L.ecsim_push_and_moments_host(self.h, n, qom, 1 if sorted else 0, *ptrs, _hptr(E, f64),
+                                                  _hptr(B, f64), dt, theta, _hptr(rho, f64), _hptr(Jhat, f64),
+                                                  _hptr(M, f64), int(accumulate)),
+               "ecsim_push_and_moments_host")
+
+    # -- knobs and instrumentation -------------------------------------------------------------
+    def set_variant(self, variant: int):
+        _check(self.L.ecsim_set_variant(self.h, variant), "ecsim_set_variant")
+
+    def set_resort_fraction(self, f: float):
+        _check(self.L.ecsim_set_resort_fraction(self.h, f), "ecsim_set_resort_fraction")
+
+    def set_fused_warps(self, w: int):
+        _check(self.L.ecsim_set_fused_warps(self.h, w), "ecsim_set_fused_warps")
+
+    def enable_timing(self, on: bool = True):
+        _check(self.L.ecsim_enable_timing(self.h, 1 if on else 0), "ecsim_enable_timing")
+
+    def kernel_ms(self) -> float:
+        ms = _c.c_float()
+        _check(self.L.ecsim_kernel_ms(self.h, _c.byref(ms)), "ecsim_kernel_ms")
+        return float(ms.value)
+
+    def launch_count(self) -> int:
+        return int(self.L.ecsim_launch_count(self.h))
+
+    def stray_count(self) -> int:
+        return int(self.L.ecsim_stray_count(self.h))
+
+    def resort_count(self) -> int:
+        return int(self.L.ecsim_resort_count(self.h))
+
+    def probe_fp64(self, iters: int = 4096):
+        tf, ms = _c.c_double(), _c.c_float()
+        _check(self.L.ecsim_probe_fp64(self.h, iters, _c.byref(tf), _c.byref(ms)), "ecsim_probe_fp64")
+        return float(tf.value), float(ms.value)
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.L.ecsim_destroy(self.h)
+            self.h = None
+            self._ws = None
+            self._keep = {}
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

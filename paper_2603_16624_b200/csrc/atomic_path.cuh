@@ -1,0 +1,133 @@
+// atomic_path.cuh -- the paper's own GPU design: one thread per particle, every deposit an atomic
+// update on the global arrays ("#pragma acc atomic update"; computeMoments L131-L141
+// followed by the mover Eq. 6-8).  Correct for ANY particle order.  In libecpush it serves as
+//   (1) ECSIM_VARIANT_ATOMIC, the in-repo prior-art timing, and
+//   (2) the stray path of the fused kernel: particles listed in `list` (those found outside the
+//       cell segment they are stored in) are pushed and deposited here.
+#pragma once
+#include "common.cuh"
+
+struct AtomicArgs {
+    Geom g;
+    uint32_t n;                 // particles (or capacity of the list)
+    const uint32_t* list;       // optional: indices to process
+    const uint32_t* list_count; // device count of valid list entries
+    double *x, *y, *z, *u, *v, *w;
+    const double* q;
+    const double *E, *B;        // [3][nodes]
+    double beta;                // q dt / (2 m) (L55)
+    double dt;
+    double *rho, *J, *M;        // any may be null
+    unsigned long long* leavers; // optional: particles whose cell changed in the push
+};
+
+template <bool USE_LIST>
+__global__ void __launch_bounds__(128)
+k_push_moments_atomic(AtomicArgs a)
+{
+    const Geom& g = a.g;
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    const size_t count = USE_LIST ? (size_t)*a.list_count : (size_t)a.n;
+    unsigned my_leavers = 0;
+    for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < count; t += stride) {
+        const size_t p = USE_LIST ? a.list[t] : t;
+        const double x = a.x[p], y = a.y[p], z = a.z[p];
+        const double vx = a.u[p], vy = a.v[p], vz = a.w[p];
+        const double q = a.q[p];
+
+        // nodes N-, N+ and the 2x2x2 linear weights (L49, L131)
+        const double sx = x * g.rdx, sy = y * g.rdy, sz = z * g.rdz;
+        const int i0 = lower_node(sx, g.nx), j0 = lower_node(sy, g.ny), k0 = lower_node(sz, g.nz);
+        const int i1 = (i0 + 1 == g.nx) ? 0 : i0 + 1;
+        const int j1 = (j0 + 1 == g.ny) ? 0 : j0 + 1;
+        const int k1 = (k0 + 1 == g.nz) ? 0 : k0 + 1;
+        const double xi = sx - i0, eta = sy - j0, zeta = sz - k0;
+        const double wx[2] = {1.0 - xi, xi}, wy[2] = {1.0 - eta, eta}, wz[2] = {1.0 - zeta, zeta};
+        double W[8];
+        long long node[8];
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+            const int ia = (c >> 2) & 1, ib = (c >> 1) & 1, ic = c & 1;
+            W[c] = (wx[ia] * wy[ib]) * wz[ic];
+            node[c] = ((long long)(ia ? i1 : i0) * g.ny + (ib ? j1 : j0)) * g.nz + (ic ? k1 : k0);
+        }
+
+        // gather E^{n+theta}, B^n (L88, L133)
+        double Ep[3] = {0, 0, 0}, Bp[3] = {0, 0, 0};
+#pragma unroll
+        for (int c = 0; c < 8; ++c)
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                Ep[d] += W[c] * __ldg(a.E + d * g.nodes + node[c]);
+                Bp[d] += W[c] * __ldg(a.B + d * g.nodes + node[c]);
+            }
+
+        // rotation matrix, Eq. (2) as nine scalars (L53, L135); (I x B) v = B x v
+        const double bx = a.beta * Bp[0], by = a.beta * Bp[1], bz = a.beta * Bp[2];
+        const double invD = 1.0 / (1.0 + (bx * bx + by * by + bz * bz));
+        double al[9];
+        al[0] = invD * (1.0 + bx * bx);
+        al[1] = invD * (bx * by + bz);
+        al[2] = invD * (bx * bz - by);
+        al[3] = invD * (bx * by - bz);
+        al[4] = invD * (1.0 + by * by);
+        al[5] = invD * (by * bz + bx);
+        al[6] = invD * (bx * bz + by);
+        al[7] = invD * (by * bz - bx);
+        al[8] = invD * (1.0 + bz * bz);
+
+        // deposits with the pre-push position and velocity (L49): rho (L147), Eq. (1), Eq. (3)
+        const double vh[3] = {al[0] * vx + al[1] * vy + al[2] * vz,
+                              al[3] * vx + al[4] * vy + al[5] * vz,
+                              al[6] * vx + al[7] * vy + al[8] * vz};
+        const double qV = q * g.invV;
+        const double qbV = qV * a.beta;
+#pragma unroll 1
+        for (int c = 0; c < 8; ++c) {
+            const long long gn = node[c];
+            const double dr = qV * W[c];
+            if (a.rho) atomicAdd(a.rho + gn, dr);
+            if (a.J) {
+                atomicAdd(a.J + 0 * g.nodes + gn, dr * vh[0]);
+                atomicAdd(a.J + 1 * g.nodes + gn, dr * vh[1]);
+                atomicAdd(a.J + 2 * g.nodes + gn, dr * vh[2]);
+            }
+            if (a.M) {
+#pragma unroll
+                for (int c2 = 0; c2 < 8; ++c2) {
+                    // neighbour slot of N' relative to N: o = (di+1)*9 + (dj+1)*3 + (dk+1)
+                    const int o = (((c2 >> 2) & 1) - ((c >> 2) & 1) + 1) * 9 +
+                                  (((c2 >> 1) & 1) - ((c >> 1) & 1) + 1) * 3 +
+                                  ((c2 & 1) - (c & 1) + 1);
+                    const double cf = qbV * (W[c] * W[c2]);
+                    double* m = a.M + ((size_t)gn * 27 + o) * 9;
+#pragma unroll
+                    for (int e = 0; e < 9; ++e) atomicAdd(m + e, cf * al[e]);
+                }
+            }
+        }
+
+        // mover, Eq. (6)-(8) with periodic wrap
+        const double tx = vx + a.beta * Ep[0], ty = vy + a.beta * Ep[1], tz = vz + a.beta * Ep[2];
+        const double vbx = al[0] * tx + al[1] * ty + al[2] * tz;
+        const double vby = al[3] * tx + al[4] * ty + al[5] * tz;
+        const double vbz = al[6] * tx + al[7] * ty + al[8] * tz;
+        const double un = 2.0 * vbx - vx, vn = 2.0 * vby - vy, wn = 2.0 * vbz - vz;
+        const double xn = wrap_periodic(x + a.dt * un, g.Lx);
+        const double yn = wrap_periodic(y + a.dt * vn, g.Ly);
+        const double zn = wrap_periodic(z + a.dt * wn, g.Lz);
+        a.u[p] = un; a.v[p] = vn; a.w[p] = wn;
+        a.x[p] = xn; a.y[p] = yn; a.z[p] = zn;
+        if (USE_LIST) {
+            my_leavers += 1;   // a stray stays outside the segment it is stored in
+        } else if (a.leavers) {
+            const int i2 = lower_node(xn * g.rdx, g.nx), j2 = lower_node(yn * g.rdy, g.ny),
+                      k2 = lower_node(zn * g.rdz, g.nz);
+            my_leavers += (i2 != i0) | (j2 != j0) | (k2 != k0);
+        }
+    }
+    if (a.leavers) {
+        my_leavers = __reduce_add_sync(0xffffffffu, my_leavers);
+        if (lane_id() == 0 && my_leavers) atomicAdd(a.leavers, (unsigned long long)my_leavers);
+    }
+}

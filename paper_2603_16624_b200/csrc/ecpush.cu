@@ -1,0 +1,685 @@
+// ecpush.cu -- C ABI of libecpush (include/ecpush.h): context, workspace, orchestration of the
+// sm_100a kernels in sort.cuh / fused.cuh / atomic_path.cuh.  Product code: no CPU fallback, no
+// code shared with oracle/.  Every entry point returns an ecsim_status and never throws.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+#include <new>
+
+#include "../../include/ecpush.h"
+#include "common.cuh"
+#include "sort.cuh"
+#include "atomic_path.cuh"
+#include "fused.cuh"
+#include "probe.cuh"
+
+// --------------------------------------------------------------------------------------------
+static thread_local char g_last_error[512] = "";
+
+static int cuda_fail(cudaError_t e, const char* what, int line)
+{
+    snprintf(g_last_error, sizeof(g_last_error), "%s failed at ecpush.cu:%d: %s (%s)", what, line,
+             cudaGetErrorString(e), cudaGetErrorName(e));
+    return ECSIM_ERR_CUDA;
+}
+#define CK(call)                                                        \
+    do {                                                                \
+        cudaError_t e__ = (call);                                       \
+        if (e__ != cudaSuccess) return cuda_fail(e__, #call, __LINE__); \
+    } while (0)
+#define CK_LAUNCH() CK(cudaGetLastError())
+
+enum SortState { ST_UNSORTED = 0, ST_DECLARED = 1, ST_SEGMENTED = 2 };
+
+struct SpeciesHost {
+    bool loaded = false;
+    int64_t n = 0;
+    double qom = 0.0;
+    double *x = nullptr, *y = nullptr, *z = nullptr, *u = nullptr, *v = nullptr, *w = nullptr, *q = nullptr;
+    int state = ST_UNSORTED;
+    bool leavers_pending = false;   // an async copy of the leaver counter is in flight
+    cudaEvent_t leavers_event = nullptr;
+};
+
+struct Workspace {
+    void* base = nullptr;
+    size_t bytes = 0;
+    int64_t n_max = 0;
+    // carved regions
+    uint32_t* start = nullptr;       // [n_species][cells+1]
+    uint32_t* count = nullptr;       // [cells]
+    uint32_t* block_sums = nullptr;  // [ceil(cells/1024)]
+    int32_t* cell = nullptr;         // [n_max]
+    uint32_t* rank = nullptr;        // [n_max]
+    uint32_t* perm = nullptr;        // [n_max]
+    double* spare = nullptr;         // [n_max]
+    uint32_t* stray_list = nullptr;  // [n_species][n_max]
+    double* AM = nullptr;            // [cells][243]
+    double* AJ = nullptr;            // [n_species][cells][32]
+    uint32_t* stray_count = nullptr; // [n_species]
+    unsigned long long* leavers = nullptr; // [n_species]
+    char* extra = nullptr;           // what is left (host-step staging)
+    size_t extra_bytes = 0;
+};
+
+struct ecsim_ctx {
+    Geom g;
+    int n_species = 0;
+    cudaStream_t stream = nullptr;
+    SpeciesHost* sp = nullptr;
+    Workspace ws;
+    int variant = ECSIM_VARIANT_FUSED;
+    double resort_fraction = 0.01;
+    int timing = 0;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    bool ev_valid = false;
+    int64_t launches = 0;
+    int sm_count = 0;
+    int fused_warps = 12;
+    unsigned long long* h_leavers = nullptr;  // pinned [n_species]
+    uint32_t* h_strays = nullptr;             // pinned [n_species]
+    int last_call_species[ECSIM_MAX_SPECIES];
+    int last_call_n = 0;
+    int64_t resorts = 0;
+};
+
+static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+struct Carver {
+    char* p;
+    size_t off = 0;
+    template <class T> T* take(size_t count)
+    {
+        T* r = p ? reinterpret_cast<T*>(p + off) : nullptr;
+        off = align_up(off + count * sizeof(T), 256);
+        return r;
+    }
+};
+
+static size_t carve(const ecsim_ctx* c, int64_t n_max, void* base, Workspace* out)
+{
+    const size_t cells = (size_t)c->g.nodes;
+    const size_t nsp = (size_t)c->n_species;
+    const size_t n = (size_t)(n_max > 0 ? n_max : 0);
+    Carver k{reinterpret_cast<char*>(base)};
+    Workspace w;
+    w.start = k.take<uint32_t>(nsp * (cells + 1));
+    w.count = k.take<uint32_t>(cells);
+    w.block_sums = k.take<uint32_t>((cells + SCAN_BLOCK - 1) / SCAN_BLOCK + 1);
+    w.cell = k.take<int32_t>(n);
+    w.rank = k.take<uint32_t>(n);
+    w.perm = k.take<uint32_t>(n);
+    w.spare = k.take<double>(n);
+    w.stray_list = k.take<uint32_t>(nsp * n);
+    w.AM = k.take<double>(cells * AM_PER_CELL);
+    w.AJ = k.take<double>(nsp * cells * AJ_PER_CELL);
+    w.stray_count = k.take<uint32_t>(nsp);
+    w.leavers = k.take<unsigned long long>(nsp);
+    if (out) {
+        w.base = base;
+        w.n_max = n_max;
+        *out = w;
+    }
+    return k.off;
+}
+
+static int grid_for(const ecsim_ctx* c, size_t work, int block, int per_sm)
+{
+    size_t blocks = (work + block - 1) / block;
+    size_t cap = (size_t)c->sm_count * per_sm;
+    if (blocks > cap) blocks = cap;
+    if (blocks < 1) blocks = 1;
+    return (int)blocks;
+}
+
+// --------------------------------------------------------------------------------------------
+extern "C" const char* ecsim_strerror(int status)
+{
+    switch (status) {
+    case ECSIM_OK: return "ok";
+    case ECSIM_ERR_INVALID_ARG: return "invalid argument";
+    case ECSIM_ERR_NOT_LOADED: return "species has no particles loaded";
+    case ECSIM_ERR_WORKSPACE: return "workspace missing or too small";
+    case ECSIM_ERR_CUDA: return "CUDA call failed (see ecsim_last_error)";
+    case ECSIM_ERR_NOMEM: return "host allocation failed";
+    default: return "unknown status";
+    }
+}
+
+extern "C" const char* ecsim_last_error(void) { return g_last_error; }
+
+extern "C" int ecsim_init_grid(ecsim_ctx** ctx, int nx, int ny, int nz, double dx, double dy, double dz,
+                               int n_species, void* cuda_stream)
+{
+    if (!ctx) return ECSIM_ERR_INVALID_ARG;
+    *ctx = nullptr;
+    if (nx < 2 || ny < 2 || nz < 2 || !(dx > 0) || !(dy > 0) || !(dz > 0) || n_species < 1 ||
+        n_species > ECSIM_MAX_SPECIES || (int64_t)nx * ny * nz > 0x7fffffffLL)
+        return ECSIM_ERR_INVALID_ARG;
+    int dev = 0;
+    CK(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    CK(cudaGetDeviceProperties(&prop, dev));
+    ecsim_ctx* c = new (std::nothrow) ecsim_ctx();
+    if (!c) return ECSIM_ERR_NOMEM;
+    c->sp = new (std::nothrow) SpeciesHost[n_species];
+    if (!c->sp) { delete c; return ECSIM_ERR_NOMEM; }
+    Geom& g = c->g;
+    g.nx = nx; g.ny = ny; g.nz = nz;
+    g.dx = dx; g.dy = dy; g.dz = dz;
+    g.rdx = 1.0 / dx; g.rdy = 1.0 / dy; g.rdz = 1.0 / dz;
+    g.Lx = nx * dx; g.Ly = ny * dy; g.Lz = nz * dz;
+    g.invV = 1.0 / (dx * dy * dz);
+    g.nodes = (long long)nx * ny * nz;
+    c->n_species = n_species;
+    c->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    c->sm_count = prop.multiProcessorCount;
+    cudaError_t e = cudaEventCreate(&c->ev0);
+    if (e == cudaSuccess) e = cudaEventCreate(&c->ev1);
+    for (int s = 0; s < n_species && e == cudaSuccess; ++s)
+        e = cudaEventCreateWithFlags(&c->sp[s].leavers_event, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaMallocHost(&c->h_leavers, sizeof(unsigned long long) * n_species);
+    if (e == cudaSuccess) e = cudaMallocHost(&c->h_strays, sizeof(uint32_t) * n_species);
+    if (e != cudaSuccess) {
+        int rc = cuda_fail(e, "context set-up", __LINE__);
+        ecsim_destroy(c);
+        return rc;
+    }
+    for (int s = 0; s < n_species; ++s) { c->h_leavers[s] = 0; c->h_strays[s] = 0; }
+    *ctx = c;
+    return ECSIM_OK;
+}
+
+extern "C" int ecsim_destroy(ecsim_ctx* c)
+{
+    if (!c) return ECSIM_OK;
+    if (c->sp) {
+        for (int s = 0; s < c->n_species; ++s)
+            if (c->sp[s].leavers_event) cudaEventDestroy(c->sp[s].leavers_event);
+        delete[] c->sp;
+    }
+    if (c->ev0) cudaEventDestroy(c->ev0);
+    if (c->ev1) cudaEventDestroy(c->ev1);
+    if (c->h_leavers) cudaFreeHost(c->h_leavers);
+    if (c->h_strays) cudaFreeHost(c->h_strays);
+    delete c;
+    return ECSIM_OK;
+}
+
+extern "C" size_t ecsim_workspace_bytes(const ecsim_ctx* c, int64_t n_particles_max)
+{
+    if (!c || n_particles_max < 0) return 0;
+    return carve(c, n_particles_max, nullptr, nullptr);
+}
+
+extern "C" int ecsim_set_workspace(ecsim_ctx* c, void* dev_ptr, size_t bytes)
+{
+    if (!c || !dev_ptr || (reinterpret_cast<uintptr_t>(dev_ptr) & 255u)) return ECSIM_ERR_INVALID_ARG;
+    // n_max = the largest particle count the buffer can serve
+    const size_t fixed = carve(c, 0, nullptr, nullptr);
+    if (bytes < fixed) return ECSIM_ERR_WORKSPACE;
+    const size_t per_particle = sizeof(int32_t) + 2 * sizeof(uint32_t) + sizeof(double) +
+                                (size_t)c->n_species * sizeof(uint32_t);
+    int64_t n_max = (int64_t)((bytes - fixed) / per_particle);
+    while (n_max > 0 && carve(c, n_max, nullptr, nullptr) > bytes) n_max -= 64;
+    if (n_max < 0) n_max = 0;
+    const size_t used = carve(c, n_max, dev_ptr, &c->ws);
+    c->ws.bytes = bytes;
+    c->ws.extra = reinterpret_cast<char*>(dev_ptr) + used;
+    c->ws.extra_bytes = bytes - used;
+    for (int s = 0; s < c->n_species; ++s)
+        if (c->sp[s].state == ST_SEGMENTED) c->sp[s].state = ST_DECLARED;  // tables lived in the old buffer
+    return ECSIM_OK;
+}
+
+static int check_species(const ecsim_ctx* c, int s)
+{
+    if (!c || s < 0 || s >= c->n_species) return ECSIM_ERR_INVALID_ARG;
+    if (!c->sp[s].loaded) return ECSIM_ERR_NOT_LOADED;
+    return ECSIM_OK;
+}
+
+static int need_workspace(const ecsim_ctx* c, int64_t n)
+{
+    if (!c->ws.base || c->ws.n_max < n) return ECSIM_ERR_WORKSPACE;
+    return ECSIM_OK;
+}
+
+extern "C" int ecsim_load_particles(ecsim_ctx* c, int s, int64_t n, double q_over_m,
+                                    double* x, double* y, double* z, double* u, double* v, double* w,
+                                    double* q, int sorted)
+{
+    if (!c || s < 0 || s >= c->n_species || n < 0 || n > 0xffffffffLL || !isfinite(q_over_m))
+        return ECSIM_ERR_INVALID_ARG;
+    if (n > 0 && (!x || !y || !z || !u || !v || !w || !q)) return ECSIM_ERR_INVALID_ARG;
+    SpeciesHost& sp = c->sp[s];
+    sp.loaded = true;
+    sp.n = n;
+    sp.qom = q_over_m;
+    sp.x = x; sp.y = y; sp.z = z; sp.u = u; sp.v = v; sp.w = w; sp.q = q;
+    sp.state = sorted ? ST_DECLARED : ST_UNSORTED;
+    sp.leavers_pending = false;
+    return ECSIM_OK;
+}
+
+// histogram of the species as stored + exclusive scan -> start table of the species
+static int histogram_and_scan(ecsim_ctx* c, int s, bool with_rank)
+{
+    SpeciesHost& sp = c->sp[s];
+    Workspace& w = c->ws;
+    const uint32_t cells = (uint32_t)c->g.nodes;
+    uint32_t* start = w.start + (size_t)s * (cells + 1);
+    CK(cudaMemsetAsync(w.count, 0, sizeof(uint32_t) * cells, c->stream));
+    c->launches++;
+    if (sp.n > 0) {
+        const int grid = grid_for(c, (size_t)sp.n, 256, 16);
+        if (with_rank)
+            k_cell_hist<true><<<grid, 256, 0, c->stream>>>(c->g, (uint32_t)sp.n, sp.x, sp.y, sp.z, w.cell, w.rank, w.count);
+        else
+            k_cell_hist<false><<<grid, 256, 0, c->stream>>>(c->g, (uint32_t)sp.n, sp.x, sp.y, sp.z, nullptr, nullptr, w.count);
+        CK_LAUNCH();
+        c->launches++;
+    }
+    const uint32_t nb = (cells + SCAN_BLOCK - 1) / SCAN_BLOCK;
+    k_scan_blocks<<<nb, SCAN_BLOCK, 0, c->stream>>>(w.count, start, w.block_sums, cells);
+    CK_LAUNCH();
+    k_scan_sums<<<1, SCAN_BLOCK, 0, c->stream>>>(w.block_sums, nb, start, cells);
+    CK_LAUNCH();
+    k_scan_add<<<nb, SCAN_BLOCK, 0, c->stream>>>(start, w.block_sums, cells);
+    CK_LAUNCH();
+    c->launches += 3;
+    return ECSIM_OK;
+}
+
+extern "C" int ecsim_build_segments(ecsim_ctx* c, int s)
+{
+    int rc = check_species(c, s);
+    if (rc) return rc;
+    rc = need_workspace(c, c->sp[s].n);
+    if (rc) return rc;
+    rc = histogram_and_scan(c, s, false);
+    if (rc) return rc;
+    c->sp[s].state = ST_SEGMENTED;
+    c->sp[s].leavers_pending = false;
+    return ECSIM_OK;
+}
+
+extern "C" int ecsim_sort_particles(ecsim_ctx* c, int s, int32_t* cell_count_out, uint32_t* perm_out)
+{
+    int rc = check_species(c, s);
+    if (rc) return rc;
+    SpeciesHost& sp = c->sp[s];
+    rc = need_workspace(c, sp.n);
+    if (rc) return rc;
+    Workspace& w = c->ws;
+    const uint32_t cells = (uint32_t)c->g.nodes;
+    const uint32_t* start = w.start + (size_t)s * (cells + 1);
+    rc = histogram_and_scan(c, s, true);
+    if (rc) return rc;
+    if (sp.n > 0) {
+        const uint32_t n = (uint32_t)sp.n;
+        const int grid = grid_for(c, (size_t)sp.n, 256, 16);
+        k_build_perm<<<grid, 256, 0, c->stream>>>(n, w.cell, w.rank, start, w.perm);
+        CK_LAUNCH();
+        c->launches++;
+        double* arrays[7] = {sp.x, sp.y, sp.z, sp.u, sp.v, sp.w, sp.q};
+        for (int a = 0; a < 7; ++a) {
+            k_gather_f64<<<grid, 256, 0, c->stream>>>(n, w.perm, arrays[a], w.spare);
+            CK_LAUNCH();
+            CK(cudaMemcpyAsync(arrays[a], w.spare, sizeof(double) * (size_t)n, cudaMemcpyDeviceToDevice, c->stream));
+            c->launches += 2;
+        }
+        if (perm_out)
+            CK(cudaMemcpyAsync(perm_out, w.perm, sizeof(uint32_t) * (size_t)n, cudaMemcpyDeviceToDevice, c->stream));
+    }
+    if (cell_count_out) {
+        k_copy_u32_to_i32<<<grid_for(c, cells, 256, 8), 256, 0, c->stream>>>(cells, w.count, cell_count_out);
+        CK_LAUNCH();
+        c->launches++;
+    }
+    sp.state = ST_SEGMENTED;
+    sp.leavers_pending = false;
+    return ECSIM_OK;
+}
+
+extern "C" int ecsim_cell_index(ecsim_ctx* c, int s, int32_t* cell_out)
+{
+    int rc = check_species(c, s);
+    if (rc) return rc;
+    if (!cell_out) return ECSIM_ERR_INVALID_ARG;
+    SpeciesHost& sp = c->sp[s];
+    if (sp.n == 0) return ECSIM_OK;
+    k_cell_index<<<grid_for(c, (size_t)sp.n, 256, 16), 256, 0, c->stream>>>(c->g, (uint32_t)sp.n, sp.x, sp.y, sp.z, cell_out);
+    CK_LAUNCH();
+    c->launches++;
+    return ECSIM_OK;
+}
+
+extern "C" int ecsim_set_variant(ecsim_ctx* c, int variant)
+{
+    if (!c || (variant != ECSIM_VARIANT_ATOMIC && variant != ECSIM_VARIANT_FUSED)) return ECSIM_ERR_INVALID_ARG;
+    c->variant = variant;
+    return ECSIM_OK;
+}
+
+extern "C" int ecsim_set_resort_fraction(ecsim_ctx* c, double fraction)
+{
+    if (!c || !(fraction >= 0.0)) return ECSIM_ERR_INVALID_ARG;
+    c->resort_fraction = fraction;
+    return ECSIM_OK;
+}
+
+extern "C" int ecsim_set_fused_warps(ecsim_ctx* c, int warps)
+{
+    if (!c || (warps != 8 && warps != 12 && warps != 16)) return ECSIM_ERR_INVALID_ARG;
+    c->fused_warps = warps;
+    return ECSIM_OK;
+}
+
+extern "C" int ecsim_enable_timing(ecsim_ctx* c, int on)
+{
+    if (!c) return ECSIM_ERR_INVALID_ARG;
+    c->timing = on ? 1 : 0;
+    c->ev_valid = false;
+    return ECSIM_OK;
+}
+
+extern "C" int ecsim_kernel_ms(ecsim_ctx* c, float* ms_out)
+{
+    if (!c || !ms_out) return ECSIM_ERR_INVALID_ARG;
+    if (!c->ev_valid) return ECSIM_ERR_NOT_LOADED;
+    CK(cudaEventSynchronize(c->ev1));
+    CK(cudaEventElapsedTime(ms_out, c->ev0, c->ev1));
+    return ECSIM_OK;
+}
+
+extern "C" int64_t ecsim_launch_count(const ecsim_ctx* c) { return c ? c->launches : 0; }
+extern "C" int64_t ecsim_resort_count(const ecsim_ctx* c) { return c ? c->resorts : 0; }
+
+extern "C" int64_t ecsim_stray_count(ecsim_ctx* c)
+{
+    if (!c || !c->ws.base || c->last_call_n == 0) return 0;
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return -1;
+    int64_t total = 0;
+    for (int i = 0; i < c->last_call_n; ++i) total += c->h_strays[c->last_call_species[i]];
+    return total;
+}
+
+template <int NW>
+static cudaError_t launch_fused(const ecsim_ctx* c, const FusedArgs& fa)
+{
+    const size_t smem = (size_t)NW * WARP_SMEM_DOUBLES * sizeof(double);
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(k_fused_push_moments<NW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    const size_t cells = (size_t)c->g.nodes;
+    size_t grid = (cells + NW - 1) / NW;
+    if (grid > (size_t)c->sm_count) grid = (size_t)c->sm_count;
+    k_fused_push_moments<NW><<<(int)grid, NW * 32, smem, c->stream>>>(fa);
+    return cudaGetLastError();
+}
+
+// One hot-path step for the listed species.  rho/J: per listed species (stride given), M shared.
+static int push_and_moments_impl(ecsim_ctx* c, int n_list, const int* list, const double* E, const double* B,
+                                 double dt, double theta, double* rho, size_t rho_stride, double* J,
+                                 size_t J_stride, double* M, int accumulate)
+{
+    if (!c || !E || !B || !(dt > 0.0) || !(theta >= 0.5 && theta <= 1.0)) return ECSIM_ERR_INVALID_ARG;
+    for (int i = 0; i < n_list; ++i) {
+        int rc = check_species(c, list[i]);
+        if (rc) return rc;
+    }
+    if (accumulate < 0 || accumulate > 2) return ECSIM_ERR_INVALID_ARG;
+    const int acc_M = accumulate != ECSIM_ACC_NONE;      // M: summed over species (L59)
+    const int acc_J = accumulate == ECSIM_ACC_ALL;       // rho/Jhat: per species unless asked (L129)
+    const Geom& g = c->g;
+    const size_t nodes = (size_t)g.nodes;
+    c->last_call_n = 0;
+
+    if (c->variant == ECSIM_VARIANT_ATOMIC) {
+        // the paper's design: zero the outputs, then one global atomic per scalar contribution
+        if (M && !acc_M) { CK(cudaMemsetAsync(M, 0, sizeof(double) * nodes * 243, c->stream)); c->launches++; }
+        if (!acc_J) {
+            for (int i = 0; i < n_list; ++i) {
+                if (rho) { CK(cudaMemsetAsync(rho + i * rho_stride, 0, sizeof(double) * nodes, c->stream)); c->launches++; }
+                if (J) { CK(cudaMemsetAsync(J + i * J_stride, 0, sizeof(double) * 3 * nodes, c->stream)); c->launches++; }
+            }
+        }
+        if (c->timing) CK(cudaEventRecord(c->ev0, c->stream));
+        for (int i = 0; i < n_list; ++i) {
+            SpeciesHost& sp = c->sp[list[i]];
+            if (sp.n == 0) continue;
+            AtomicArgs a;
+            a.g = g; a.n = (uint32_t)sp.n; a.list = nullptr; a.list_count = nullptr;
+            a.x = sp.x; a.y = sp.y; a.z = sp.z; a.u = sp.u; a.v = sp.v; a.w = sp.w; a.q = sp.q;
+            a.E = E; a.B = B; a.beta = sp.qom * dt / 2.0; a.dt = dt;
+            a.rho = rho ? rho + i * rho_stride : nullptr;
+            a.J = J ? J + i * J_stride : nullptr;
+            a.M = M; a.leavers = nullptr;
+            k_push_moments_atomic<false><<<grid_for(c, (size_t)sp.n, 128, 16), 128, 0, c->stream>>>(a);
+            CK_LAUNCH();
+            c->launches++;
+            sp.state = ST_UNSORTED;
+        }
+        if (c->timing) { CK(cudaEventRecord(c->ev1, c->stream)); c->ev_valid = true; }
+        return ECSIM_OK;
+    }
+
+    // ---- fused variant ----
+    int64_t n_need = 0;
+    for (int i = 0; i < n_list; ++i) n_need = c->sp[list[i]].n > n_need ? c->sp[list[i]].n : n_need;
+    int rc = need_workspace(c, n_need);
+    if (rc) return rc;
+    Workspace& w = c->ws;
+    const uint32_t cells = (uint32_t)nodes;
+
+    // segment tables: build, or re-sort when too many particles left their cell in the last push
+    for (int i = 0; i < n_list; ++i) {
+        const int s = list[i];
+        SpeciesHost& sp = c->sp[s];
+        if (sp.state == ST_SEGMENTED && sp.leavers_pending) {
+            CK(cudaEventSynchronize(sp.leavers_event));
+            sp.leavers_pending = false;
+            if ((double)c->h_leavers[s] > c->resort_fraction * (double)sp.n) sp.state = ST_UNSORTED;
+        }
+        if (sp.state == ST_UNSORTED) {
+            rc = ecsim_sort_particles(c, s, nullptr, nullptr);
+            c->resorts++;
+        } else if (sp.state == ST_DECLARED) {
+            rc = ecsim_build_segments(c, s);
+        }
+        if (rc) return rc;
+    }
+
+    CK(cudaMemsetAsync(w.stray_count, 0, sizeof(uint32_t) * c->n_species, c->stream));
+    CK(cudaMemsetAsync(w.leavers, 0, sizeof(unsigned long long) * c->n_species, c->stream));
+    c->launches += 2;
+
+    FusedArgs fa;
+    fa.g = g; fa.n_species = n_list; fa.E = E; fa.B = B; fa.dt = dt; fa.AM = w.AM;
+    for (int i = 0; i < n_list; ++i) {
+        const int s = list[i];
+        SpeciesHost& sp = c->sp[s];
+        SpeciesDev& d = fa.sp[i];
+        d.start = w.start + (size_t)s * (cells + 1);
+        d.x = sp.x; d.y = sp.y; d.z = sp.z; d.u = sp.u; d.v = sp.v; d.w = sp.w; d.q = sp.q;
+        d.beta = sp.qom * dt / 2.0;
+        d.AJ = w.AJ + (size_t)s * cells * AJ_PER_CELL;
+        d.stray_list = w.stray_list + (size_t)s * (size_t)w.n_max;
+        d.stray_count = w.stray_count + s;
+        d.leavers = w.leavers + s;
+    }
+    if (c->timing) CK(cudaEventRecord(c->ev0, c->stream));
+    cudaError_t e;
+    if (c->fused_warps == 8) e = launch_fused<8>(c, fa);
+    else if (c->fused_warps == 16) e = launch_fused<16>(c, fa);
+    else e = launch_fused<12>(c, fa);
+    if (e != cudaSuccess) return cuda_fail(e, "k_fused_push_moments launch", __LINE__);
+    c->launches++;
+    if (c->timing) { CK(cudaEventRecord(c->ev1, c->stream)); c->ev_valid = true; }
+
+    // per-cell classes -> node arrays
+    if (M) {
+        ExpandArgs ea{g, w.AM, M, acc_M};
+        const long long blocks = (g.nodes + EXPAND_NODES - 1) / EXPAND_NODES;
+        k_expand_M<<<(unsigned)blocks, 256, 0, c->stream>>>(ea);
+        CK_LAUNCH();
+        c->launches++;
+    }
+    for (int i = 0; i < n_list; ++i) {
+        if (!rho && !J) break;
+        ExpandJArgs ja{g, fa.sp[i].AJ, rho ? rho + i * rho_stride : nullptr, J ? J + i * J_stride : nullptr, acc_J};
+        k_expand_rhoJ<<<(unsigned)((g.nodes + 255) / 256), 256, 0, c->stream>>>(ja);
+        CK_LAUNCH();
+        c->launches++;
+    }
+    // strays: the atomic path adds them to the node arrays (after the expansion wrote them)
+    for (int i = 0; i < n_list; ++i) {
+        const int s = list[i];
+        SpeciesHost& sp = c->sp[s];
+        if (sp.n > 0) {
+            AtomicArgs a;
+            a.g = g; a.n = (uint32_t)sp.n; a.list = fa.sp[i].stray_list; a.list_count = fa.sp[i].stray_count;
+            a.x = sp.x; a.y = sp.y; a.z = sp.z; a.u = sp.u; a.v = sp.v; a.w = sp.w; a.q = sp.q;
+            a.E = E; a.B = B; a.beta = fa.sp[i].beta; a.dt = dt;
+            a.rho = rho ? rho + i * rho_stride : nullptr;
+            a.J = J ? J + i * J_stride : nullptr;
+            a.M = M; a.leavers = fa.sp[i].leavers;
+            k_push_moments_atomic<true><<<c->sm_count * 2, 128, 0, c->stream>>>(a);
+            CK_LAUNCH();
+            c->launches++;
+        }
+        CK(cudaMemcpyAsync(c->h_leavers + s, w.leavers + s, sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+        CK(cudaMemcpyAsync(c->h_strays + s, w.stray_count + s, sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream));
+        CK(cudaEventRecord(sp.leavers_event, c->stream));
+        sp.leavers_pending = true;
+        c->last_call_species[c->last_call_n++] = s;
+    }
+    return ECSIM_OK;
+}
+
+extern "C" int ecsim_push_and_moments(ecsim_ctx* c, int species, const double* E_theta, const double* B,
+                                      double dt, double theta, double* rho, double* Jhat, double* M, int accumulate)
+{
+    return push_and_moments_impl(c, 1, &species, E_theta, B, dt, theta, rho, 0, Jhat, 0, M, accumulate);
+}
+
+extern "C" int ecsim_push_and_moments_all(ecsim_ctx* c, const double* E_theta, const double* B, double dt,
+                                          double theta, double* rho, double* Jhat, double* M, int accumulate)
+{
+    if (!c) return ECSIM_ERR_INVALID_ARG;
+    int list[ECSIM_MAX_SPECIES];
+    for (int s = 0; s < c->n_species; ++s) list[s] = s;
+    const size_t nodes = (size_t)c->g.nodes;
+    return push_and_moments_impl(c, c->n_species, list, E_theta, B, dt, theta, rho, nodes, Jhat, 3 * nodes, M, accumulate);
+}
+
+// --------------------------------------------------------------------------------------------
+// Host-buffer step (the end-to-end path): stage in the workspace tail, run, copy back, synchronise.
+static size_t host_step_extra(const ecsim_ctx* c, int64_t n)
+{
+    const size_t nodes = (size_t)c->g.nodes;
+    return align_up(sizeof(double) * 7 * (size_t)n, 256) + align_up(sizeof(double) * 6 * nodes, 256) +
+           align_up(sizeof(double) * 4 * nodes, 256) + align_up(sizeof(double) * 243 * nodes, 256);
+}
+
+extern "C" size_t ecsim_host_step_workspace_bytes(const ecsim_ctx* c, int64_t n_particles)
+{
+    if (!c || n_particles < 0) return 0;
+    return ecsim_workspace_bytes(c, n_particles) + host_step_extra(c, n_particles);
+}
+
+extern "C" int ecsim_push_and_moments_host(ecsim_ctx* c, int64_t n, double q_over_m, int sorted,
+                                           double* x, double* y, double* z, double* u, double* v, double* w,
+                                           const double* q, const double* E_theta, const double* B,
+                                           double dt, double theta, double* rho, double* Jhat, double* M, int accumulate)
+{
+    if (!c || n < 0 || !x || !y || !z || !u || !v || !w || !q || !E_theta || !B) return ECSIM_ERR_INVALID_ARG;
+    if (!c->ws.base || c->ws.bytes < ecsim_host_step_workspace_bytes(c, n)) return ECSIM_ERR_WORKSPACE;
+    // re-carve so that exactly n particles are served and the tail is free for staging
+    Workspace keep = c->ws;
+    const size_t used = carve(c, n, keep.base, &c->ws);
+    c->ws.bytes = keep.bytes;
+    char* tail = reinterpret_cast<char*>(keep.base) + used;
+    const size_t nodes = (size_t)c->g.nodes;
+    const size_t pn = (size_t)n;
+    double* dpart = reinterpret_cast<double*>(tail);
+    tail += align_up(sizeof(double) * 7 * pn, 256);
+    double* dE = reinterpret_cast<double*>(tail);
+    double* dB = dE + 3 * nodes;
+    tail += align_up(sizeof(double) * 6 * nodes, 256);
+    double* drho = reinterpret_cast<double*>(tail);
+    double* dJ = drho + nodes;
+    tail += align_up(sizeof(double) * 4 * nodes, 256);
+    double* dM = reinterpret_cast<double*>(tail);
+    cudaStream_t st = c->stream;
+    double* hp[7] = {x, y, z, u, v, w, const_cast<double*>(q)};
+    for (int a = 0; a < 7; ++a)
+        CK(cudaMemcpyAsync(dpart + a * pn, hp[a], sizeof(double) * pn, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(dE, E_theta, sizeof(double) * 3 * nodes, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(dB, B, sizeof(double) * 3 * nodes, cudaMemcpyHostToDevice, st));
+    if (accumulate == ECSIM_ACC_ALL) {
+        if (rho) CK(cudaMemcpyAsync(drho, rho, sizeof(double) * nodes, cudaMemcpyHostToDevice, st));
+        if (Jhat) CK(cudaMemcpyAsync(dJ, Jhat, sizeof(double) * 3 * nodes, cudaMemcpyHostToDevice, st));
+    }
+    if (accumulate != ECSIM_ACC_NONE && M)
+        CK(cudaMemcpyAsync(dM, M, sizeof(double) * 243 * nodes, cudaMemcpyHostToDevice, st));
+    SpeciesHost saved = c->sp[0];
+    int rc = ecsim_load_particles(c, 0, n, q_over_m, dpart, dpart + pn, dpart + 2 * pn, dpart + 3 * pn,
+                                  dpart + 4 * pn, dpart + 5 * pn, dpart + 6 * pn, sorted);
+    const int sp0 = 0;
+    if (rc == ECSIM_OK)
+        rc = push_and_moments_impl(c, 1, &sp0, dE, dB, dt, theta, rho ? drho : nullptr, 0, Jhat ? dJ : nullptr, 0,
+                                   M ? dM : nullptr, accumulate);
+    if (rc == ECSIM_OK) {
+        for (int a = 0; a < 6; ++a)
+            CK(cudaMemcpyAsync(hp[a], dpart + a * pn, sizeof(double) * pn, cudaMemcpyDeviceToHost, st));
+        if (rho) CK(cudaMemcpyAsync(rho, drho, sizeof(double) * nodes, cudaMemcpyDeviceToHost, st));
+        if (Jhat) CK(cudaMemcpyAsync(Jhat, dJ, sizeof(double) * 3 * nodes, cudaMemcpyDeviceToHost, st));
+        if (M) CK(cudaMemcpyAsync(M, dM, sizeof(double) * 243 * nodes, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+    }
+    // restore the caller's species 0 and the full carve
+    cudaEvent_t ev = c->sp[0].leavers_event;
+    c->sp[0] = saved;
+    c->sp[0].leavers_event = ev;
+    c->sp[0].leavers_pending = false;
+    if (c->sp[0].state == ST_SEGMENTED) c->sp[0].state = ST_DECLARED;
+    const size_t used2 = carve(c, keep.n_max, keep.base, &c->ws);
+    c->ws.bytes = keep.bytes;
+    c->ws.extra = reinterpret_cast<char*>(keep.base) + used2;
+    c->ws.extra_bytes = keep.bytes - used2;
+    for (int s = 1; s < c->n_species; ++s)
+        if (c->sp[s].state == ST_SEGMENTED) c->sp[s].state = ST_DECLARED;
+    return rc;
+}
+
+// --------------------------------------------------------------------------------------------
+// Device probes used by bench.py for the roofline denominators (not part of the hot path).
+extern "C" int ecsim_probe_fp64(ecsim_ctx* c, int iters, double* tflops_out, float* ms_out)
+{
+    if (!c || iters < 1 || !tflops_out) return ECSIM_ERR_INVALID_ARG;
+    double* sink = nullptr;
+    CK(cudaMalloc(&sink, sizeof(double) * 1024));
+    const int blocks = c->sm_count * 8, threads = 256;
+    k_probe_dfma<<<blocks, threads, 0, c->stream>>>(sink, 16, 1.0);   // warm-up
+    CK_LAUNCH();
+    CK(cudaEventRecord(c->ev0, c->stream));
+    k_probe_dfma<<<blocks, threads, 0, c->stream>>>(sink, iters, 1.0);
+    CK_LAUNCH();
+    CK(cudaEventRecord(c->ev1, c->stream));
+    CK(cudaEventSynchronize(c->ev1));
+    float ms = 0.f;
+    CK(cudaEventElapsedTime(&ms, c->ev0, c->ev1));
+    CK(cudaFree(sink));
+    c->ev_valid = false;
+    const double flops = 2.0 * PROBE_CHAINS * PROBE_UNROLL * (double)iters * blocks * threads;
+    *tflops_out = flops / (ms * 1e-3) * 1e-12;
+    if (ms_out) *ms_out = ms;
+    return ECSIM_OK;
+}
