@@ -222,9 +222,15 @@ extern "C" int ecsim_set_workspace(ecsim_ctx* c, void* dev_ptr, size_t bytes)
     if (bytes < fixed) return ECSIM_ERR_WORKSPACE;
     const size_t per_particle = sizeof(int32_t) + 2 * sizeof(uint32_t) + sizeof(double) +
                                 (size_t)c->n_species * sizeof(uint32_t);
-    int64_t n_max = (int64_t)((bytes - fixed) / per_particle);
-    while (n_max > 0 && carve(c, n_max, nullptr, nullptr) > bytes) n_max -= 64;
-    if (n_max < 0) n_max = 0;
+    // carve() is monotone in n: bisect for the largest n that fits (the per-array 256-byte rounding
+    // makes a closed form off by a few particles either way)
+    int64_t lo = 0, hi = (int64_t)((bytes - fixed) / per_particle) + 1;
+    if (hi > 0xffffffffLL) hi = 0xffffffffLL;
+    while (lo < hi) {
+        const int64_t mid = lo + (hi - lo + 1) / 2;
+        if (carve(c, mid, nullptr, nullptr) <= bytes) lo = mid; else hi = mid - 1;
+    }
+    int64_t n_max = lo;
     const size_t used = carve(c, n_max, dev_ptr, &c->ws);
     c->ws.bytes = bytes;
     c->ws.extra = reinterpret_cast<char*>(dev_ptr) + used;
