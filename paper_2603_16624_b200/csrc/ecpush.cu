@@ -508,6 +508,8 @@ static int push_and_moments_impl(ecsim_ctx* c, int n_list, const int* list, cons
 
     FusedArgs fa;
     fa.g = g; fa.n_species = n_list; fa.E = E; fa.B = B; fa.dt = dt; fa.AM = w.AM;
+    fa.weight_total = (unsigned long long)CELL_WEIGHT * cells;
+    for (int i = 0; i < n_list; ++i) fa.weight_total += (unsigned long long)c->sp[list[i]].n;
     for (int i = 0; i < n_list; ++i) {
         const int s = list[i];
         SpeciesHost& sp = c->sp[s];
@@ -532,7 +534,7 @@ static int push_and_moments_impl(ecsim_ctx* c, int n_list, const int* list, cons
     // per-cell classes -> node arrays
     if (M) {
         ExpandArgs ea{g, w.AM, M, acc_M};
-        const long long blocks = (g.nodes + EXPAND_NODES - 1) / EXPAND_NODES;
+        const long long blocks = (long long)g.nx * g.ny * ((g.nz + EXPAND_Z - 1) / EXPAND_Z);
         k_expand_M<<<(unsigned)blocks, 256, 0, c->stream>>>(ea);
         CK_LAUNCH();
         c->launches++;
