@@ -12,7 +12,8 @@
 #include "common.cuh"
 #include "sort.cuh"
 #include "atomic_path.cuh"
-#include "fused.cuh"
+#include "fused_mma.cuh"
+#include "expand.cuh"
 #include "probe.cuh"
 
 // --------------------------------------------------------------------------------------------
@@ -77,7 +78,7 @@ struct ecsim_ctx {
     bool ev_valid = false;
     int64_t launches = 0;
     int sm_count = 0;
-    int fused_warps = 12;
+    int fused_warps = 16;
     unsigned long long* h_leavers = nullptr;  // pinned [n_species]
     uint32_t* h_strays = nullptr;             // pinned [n_species]
     int last_call_species[ECSIM_MAX_SPECIES];
@@ -525,8 +526,8 @@ static int push_and_moments_impl(ecsim_ctx* c, int n_list, const int* list, cons
     if (c->timing) CK(cudaEventRecord(c->ev0, c->stream));
     cudaError_t e;
     if (c->fused_warps == 8) e = launch_fused<8>(c, fa);
-    else if (c->fused_warps == 16) e = launch_fused<16>(c, fa);
-    else e = launch_fused<12>(c, fa);
+    else if (c->fused_warps == 12) e = launch_fused<12>(c, fa);
+    else e = launch_fused<16>(c, fa);
     if (e != cudaSuccess) return cuda_fail(e, "k_fused_push_moments launch", __LINE__);
     c->launches++;
     if (c->timing) { CK(cudaEventRecord(c->ev1, c->stream)); c->ev_valid = true; }

@@ -1,0 +1,443 @@
+// fused_mma.cuh -- the fused gather / push / deposit kernel for cell-sorted particles
+// (SURVEY §8 rows a1-a9), version 3: the per-cell pre-reduction runs on the FP64 matrix path.
+//
+// Design:
+//   * One FP64 pipe bounds this path.  DFMA and DMMA share it (measured:
+//     34.1 / 37.1 / 32-33 TFLOP/s alone / alone / mixed), but one `mma.sync.m8n8k4.f64` carries 256
+//     FMAs in one issue slot with two operand registers per lane, where 256 DFMA-FMAs need 8 issue
+//     slots and, as rank-1 updates, ~100 operand doubles from shared memory.  Version 2 (DFMA) ran
+//     at 91 % of the shared-memory wavefront peak and 42 % of the FP64 pipe (profiles/r01a).
+//   * One warp owns a contiguous range of cells, chosen from the segment tables so that every warp
+//     of the grid gets the same number of particles (+ a per-cell weight): a particle-balanced
+//     schedule that also serves non-uniform loads (Harris sheet).
+//   * Per cell, all particles of all species of the call stream through the warp in batches of 32.
+//   * Phase 1, lane = particle, branch-free: CIC weights (L49, L131), gather of E^{n+theta}, B^n
+//     from the cell's 8 corner nodes staged in shared memory (L88, L133), alpha_p as nine scalars
+//     (Eq. 2), push (Eq. 6-8), and the per-particle factors of the deposits,
+//     written TRANSPOSED ([value][particle]) to a per-warp staging tile in shared memory:
+//         c[27]     = q/V * px[kx] py[ky] pz[kz],   p?[0..2] = (w0^2, w0 w1, w1^2)
+//         b[13]     = beta*alpha[0..7] | 1, (alpha v^n)[0..2], beta*alpha[8]
+//     Only 27 distinct products W_pN W_pN' exist per particle (three per axis), so the 8x8 = 64
+//     (node, neighbour) pairs of Eq. (3) collapse onto 27 "classes" per cell; and because
+//     sum_N' W_pN' = 1, W_pN itself is the sum of the 8 classes that pair corner N with any N':
+//     rho and Jhat (Eq. 1) come out of the same class sums.  Lanes without a particle (ragged
+//     tail, strays) run the same code with q = 0, so their columns hold zeros.
+//   * Phase 2, the pre-reduction of same-cell particles (north-star (b)) as a tall-skinny
+//     contraction over the particle index:  C[class][col] += sum_p c[class](p) * b[col](p),
+//     32 x 16 padded from 27 x 13, as 4 x 2 tiles of m8n8k4 DMMA per group of 4 particles.  Lane
+//     (r = lane/4, k = lane%4) reads c[8mt + r] and b[8nt + r] of particle 4g + k: 6 conflict-free
+//     LDS.64 per 8 DMMA.  The accumulators are 16 doubles per lane.
+//   * At the end of a species in a cell the rho/Jhat columns are folded to the 8 corners (through
+//     shared memory) and written to AJ[species][cell][8][4]; at the end of a cell the mass-matrix
+//     columns are written straight from the fragments, coalesced, to AM[cell][288].  No atomics;
+//     the result is deterministic for a given particle order.
+//   * k_expand_* (expand.cuh) then build the node arrays.
+//   * A particle found outside the cell whose segment it is stored in (a "stray") is skipped here,
+//     listed, and handled by the atomic path afterwards.
+#pragma once
+#include "common.cuh"
+
+constexpr int ST_PITCH = 36;     // doubles per staging row: 32 particles + 4 (pitch = 4 mod 16: LDS.64 conflict-free)
+constexpr int ROW_C = 0;         // rows 0..26: the 27 classes, class = kx*9 + ky*3 + kz
+constexpr int ROW_B = 27;        // rows 27..34: beta*alpha[0..7]; 35: 1; 36..38: alpha v^n; 39: beta*alpha[8]; 40..42: zero
+constexpr int ST_ROWS = 43;      // A tile 3 reads rows 24..31 (27..31 = finite junk for the 5 unused classes)
+constexpr int FLD_DOUBLES = 48;  // 8 corners x (Ex,Ey,Ez,Bx,By,Bz)
+constexpr int WARP_SMEM_DOUBLES = ST_ROWS * ST_PITCH + FLD_DOUBLES;
+constexpr int AM_PER_CELL = 288; // [4 m-tiles][8 classes][8 alpha entries] + [32 classes] alpha[8]
+constexpr int AM_A8 = 256;
+constexpr int AJ_PER_CELL = 32;
+constexpr unsigned CELL_WEIGHT = 8;   // schedule weight of a cell, in particles
+
+struct SpeciesDev {
+    const uint32_t* start;   // [cells+1] segment table
+    double *x, *y, *z, *u, *v, *w;
+    const double* q;
+    double beta;             // q dt/(2m) (L55)
+    double* AJ;              // [cells][8][4]: rho, Jx, Jy, Jz per corner
+    uint32_t* stray_list;
+    uint32_t* stray_count;
+    unsigned long long* leavers;
+};
+
+struct FusedArgs {
+    Geom g;
+    int n_species;
+    const double *E, *B;
+    double dt;
+    double* AM;                      // [cells][AM_PER_CELL]
+    unsigned long long weight_total; // sum of particles of the listed species + CELL_WEIGHT * cells
+    SpeciesDev sp[ECSIM_MAX_SPECIES];
+};
+
+__device__ __forceinline__ bool in_unit_interval(double t)
+{
+    // t in [+0, 1): sign clear and exponent below that of 1.0 (NaN and negatives fail)
+    return (unsigned)__double2hiint(t) < 0x3FF00000u;
+}
+
+// Periodic wrap with an integer fast-path test: for x >= +0 the order of doubles is the order of
+// their bit patterns, so "0 <= x < L" is one unsigned 64-bit compare (negatives and NaN fail it).
+__device__ __forceinline__ double wrap_fast(double x, double L)
+{
+    if ((unsigned long long)__double_as_longlong(x) < (unsigned long long)__double_as_longlong(L)) return x;
+    return wrap_periodic(x, L);
+}
+
+// D(8x8) += A(8x4) * B(4x8) in FP64.  Lane l holds A[l/4][l%4], B[l%4][l/4], D[l/4][2(l%4) + {0,1}].
+__device__ __forceinline__ void dmma_m8n8k4(double2& d, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(d.x), "+d"(d.y) : "d"(a), "d"(b));
+}
+
+// First cell of warp w's range: smallest c with  CELL_WEIGHT*c + sum_s start_s[c] >= w/W of the total.
+__device__ __forceinline__ uint32_t range_bound(const FusedArgs& a, uint32_t w, uint32_t W)
+{
+    const uint32_t cells = (uint32_t)a.g.nodes;
+    if (w == 0) return 0;
+    if (w >= W) return cells;
+    const unsigned long long target = a.weight_total / W * w + (a.weight_total % W) * w / W;
+    uint32_t lo = 0, hi = cells;
+    while (lo < hi) {
+        const uint32_t mid = lo + (hi - lo) / 2;
+        unsigned long long f = (unsigned long long)CELL_WEIGHT * mid;
+        for (int s = 0; s < a.n_species; ++s) f += __ldg(a.sp[s].start + mid);
+        if (f >= target) hi = mid; else lo = mid + 1;
+    }
+    return lo;
+}
+
+struct ParticleRegs { double x, y, z, u, v, w, q; };
+
+__device__ __forceinline__ void load_batch(const SpeciesDev& sp, uint32_t p0, int nb, int lane, ParticleRegs& r)
+{
+    if (lane < nb) {
+        const uint32_t p = p0 + lane;
+        r.x = sp.x[p]; r.y = sp.y[p]; r.z = sp.z[p];
+        r.u = sp.u[p]; r.v = sp.v[p]; r.w = sp.w[p];
+        r.q = __ldg(sp.q + p);
+    }
+}
+
+// Phase 1 for one lane: returns true if the lane holds a stray.  `st` = staging tile + lane (the
+// lane's column), `fld` = the cell's corner fields, (dci,dcj,dck) = the cell's integer coordinates.
+__device__ __forceinline__ bool phase1(const Geom& g, const SpeciesDev& sp, const ParticleRegs& r, bool active,
+                                       uint32_t p, double beta, double dt, double dci, double dcj, double dck,
+                                       const double* __restrict__ fld, double* __restrict__ st, unsigned& leavers)
+{
+    // weights relative to the warp's cell; outside [0,1) => not in this cell
+    double xi = r.x * g.rdx - dci, eta = r.y * g.rdy - dcj, zeta = r.z * g.rdz - dck;
+    const bool inside = active && in_unit_interval(xi) && in_unit_interval(eta) && in_unit_interval(zeta);
+    // lanes without a particle of this cell compute on harmless numbers with zero charge
+    if (!inside) { xi = 0.5; eta = 0.5; zeta = 0.5; }
+    const double vx = inside ? r.u : 0.0, vy = inside ? r.v : 0.0, vz = inside ? r.w : 0.0;
+    const double q = inside ? r.q : 0.0;
+    const double wx0 = 1.0 - xi, wy0 = 1.0 - eta, wz0 = 1.0 - zeta;
+    double Ex = 0, Ey = 0, Ez = 0, Bx = 0, By = 0, Bz = 0;
+    {
+        const double w00 = wx0 * wy0, w01 = wx0 * eta, w10 = xi * wy0, w11 = xi * eta;
+        const double W[8] = {w00 * wz0, w00 * zeta, w01 * wz0, w01 * zeta, w10 * wz0, w10 * zeta, w11 * wz0, w11 * zeta};
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const double2 f0 = *reinterpret_cast<const double2*>(fld + k * 6);
+            const double2 f1 = *reinterpret_cast<const double2*>(fld + k * 6 + 2);
+            const double2 f2 = *reinterpret_cast<const double2*>(fld + k * 6 + 4);
+            Ex = fma(W[k], f0.x, Ex); Ey = fma(W[k], f0.y, Ey); Ez = fma(W[k], f1.x, Ez);
+            Bx = fma(W[k], f1.y, Bx); By = fma(W[k], f2.x, By); Bz = fma(W[k], f2.y, Bz);
+        }
+    }
+    // alpha_p, Eq. (2): (I x B) v = B x v, b = beta B_p;  alpha = (I + [b]x)^-1
+    const double bx = beta * Bx, by = beta * By, bz = beta * Bz;
+    const double invD = 1.0 / (1.0 + (bx * bx + by * by + bz * bz));
+    const double sx = invD * bx, sy = invD * by, sz = invD * bz;
+    const double a00 = fma(bx, sx, invD), a01 = fma(bx, sy, sz), a02 = fma(bx, sz, -sy);
+    const double a10 = fma(by, sx, -sz), a11 = fma(by, sy, invD), a12 = fma(by, sz, sx);
+    const double a20 = fma(bz, sx, sy), a21 = fma(bz, sy, -sx), a22 = fma(bz, sz, invD);
+    // deposit factors (pre-push x and v, L49): B operand of the contraction
+    double* sb = st + ROW_B * ST_PITCH;
+    sb[0 * ST_PITCH] = beta * a00; sb[1 * ST_PITCH] = beta * a01; sb[2 * ST_PITCH] = beta * a02;
+    sb[3 * ST_PITCH] = beta * a10; sb[4 * ST_PITCH] = beta * a11; sb[5 * ST_PITCH] = beta * a12;
+    sb[6 * ST_PITCH] = beta * a20; sb[7 * ST_PITCH] = beta * a21; sb[12 * ST_PITCH] = beta * a22;
+    sb[9 * ST_PITCH] = a00 * vx + a01 * vy + a02 * vz;
+    sb[10 * ST_PITCH] = a10 * vx + a11 * vy + a12 * vz;
+    sb[11 * ST_PITCH] = a20 * vx + a21 * vy + a22 * vz;
+    {
+        // A operand, 27 classes: q/V * px[kx] * py[ky] * pz[kz]
+        const double qV = q * g.invV;
+        const double qx0 = qV * wx0, qx1 = qV * xi;
+        const double px[3] = {qx0 * wx0, qx0 * xi, qx1 * xi};
+        const double py[3] = {wy0 * wy0, wy0 * eta, eta * eta};
+        const double pz0 = wz0 * wz0, pz1 = wz0 * zeta, pz2 = zeta * zeta;
+#pragma unroll
+        for (int kx = 0; kx < 3; ++kx)
+#pragma unroll
+            for (int ky = 0; ky < 3; ++ky) {
+                const double pxy = px[kx] * py[ky];
+                double* sc = st + (ROW_C + (kx * 3 + ky) * 3) * ST_PITCH;
+                sc[0] = pxy * pz0; sc[ST_PITCH] = pxy * pz1; sc[2 * ST_PITCH] = pxy * pz2;
+            }
+    }
+    // mover, Eq. (6)-(8)
+    const double tx = fma(beta, Ex, vx), ty = fma(beta, Ey, vy), tz = fma(beta, Ez, vz);
+    const double vbx = a00 * tx + a01 * ty + a02 * tz;
+    const double vby = a10 * tx + a11 * ty + a12 * tz;
+    const double vbz = a20 * tx + a21 * ty + a22 * tz;
+    const double un = 2.0 * vbx - vx, vn = 2.0 * vby - vy, wn = 2.0 * vbz - vz;
+    if (inside) {
+        const double xn = wrap_fast(fma(dt, un, r.x), g.Lx);
+        const double yn = wrap_fast(fma(dt, vn, r.y), g.Ly);
+        const double zn = wrap_fast(fma(dt, wn, r.z), g.Lz);
+        sp.u[p] = un; sp.v[p] = vn; sp.w[p] = wn;
+        sp.x[p] = xn; sp.y[p] = yn; sp.z[p] = zn;
+        const bool stays = in_unit_interval(xn * g.rdx - dci) && in_unit_interval(yn * g.rdy - dcj) &&
+                           in_unit_interval(zn * g.rdz - dck);
+        leavers += stays ? 0u : 1u;
+    }
+    return active && !inside;
+}
+
+template <int NW>
+__global__ void __launch_bounds__(NW * 32, 1)
+k_fused_push_moments(const __grid_constant__ FusedArgs a)
+{
+    extern __shared__ __align__(16) double smem[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double* stg = smem + (size_t)warp * WARP_SMEM_DOUBLES;
+    double* fld = stg + ST_ROWS * ST_PITCH;
+    for (int t = lane; t < WARP_SMEM_DOUBLES; t += 32) stg[t] = 0.0;
+    __syncwarp();
+    for (int t = lane; t < ST_PITCH; t += 32) stg[(ROW_B + 8) * ST_PITCH + t] = 1.0;   // the rho column of b
+    __syncwarp();
+
+    const Geom& g = a.g;
+    const int nsp = a.n_species;
+    const double dt = a.dt;
+    const uint32_t W = gridDim.x * NW, wid = blockIdx.x * NW + warp;
+    const uint32_t c_lo = range_bound(a, wid, W), c_hi = range_bound(a, wid + 1, W);
+    if (c_lo >= c_hi) return;
+
+    // lane roles of phase 2: row r of the A / B tiles, particle k of a group of four
+    const int fr = lane >> 2, fk = lane & 3;
+    const double* frag = stg + fr * ST_PITCH + fk;
+    double* stcol = stg + lane;
+
+    // field staging: lane t and t+32 (< 48) hold corner t/6, component t%6 of the next cell
+    const int fc0 = lane / 6, fk0 = lane - fc0 * 6;
+    const int fc1 = (lane + 32) / 6, fk1 = (lane + 32) - fc1 * 6;
+    const double* fsrc0 = fk0 < 3 ? a.E + (size_t)fk0 * g.nodes : a.B + (size_t)(fk0 - 3) * g.nodes;
+    const double* fsrc1 = fk1 < 3 ? a.E + (size_t)fk1 * g.nodes : a.B + (size_t)(fk1 - 3) * g.nodes;
+    auto load_fields = [&](int ci, int cj, int ck, double& f0, double& f1) {
+        {
+            int ii = ci + ((fc0 >> 2) & 1); if (ii == g.nx) ii = 0;
+            int jj = cj + ((fc0 >> 1) & 1); if (jj == g.ny) jj = 0;
+            int kk = ck + (fc0 & 1);        if (kk == g.nz) kk = 0;
+            f0 = __ldg(fsrc0 + ((long long)ii * g.ny + jj) * g.nz + kk);
+        }
+        if (lane < FLD_DOUBLES - 32) {
+            int ii = ci + ((fc1 >> 2) & 1); if (ii == g.nx) ii = 0;
+            int jj = cj + ((fc1 >> 1) & 1); if (jj == g.ny) jj = 0;
+            int kk = ck + (fc1 & 1);        if (kk == g.nz) kk = 0;
+            f1 = __ldg(fsrc1 + ((long long)ii * g.ny + jj) * g.nz + kk);
+        }
+    };
+
+    // cell coordinates of the first cell (one division per warp; then incremented)
+    int ck = (int)(c_lo % (uint32_t)g.nz);
+    int cj = (int)((c_lo / (uint32_t)g.nz) % (uint32_t)g.ny);
+    int ci = (int)(c_lo / ((uint32_t)g.nz * (uint32_t)g.ny));
+
+    // segment registers of lane s < nsp: start_s[c], start_s[c+1], start_s[c+2]
+    uint32_t sb = 0, se = 0, sn = 0;
+    const uint32_t* my_start = a.sp[lane < nsp ? lane : 0].start;
+    if (lane < nsp) {
+        sb = __ldg(my_start + c_lo);
+        se = __ldg(my_start + c_lo + 1);
+        if (c_lo + 1 < c_hi) sn = __ldg(my_start + c_lo + 2);
+    }
+    double f0 = 0.0, f1 = 0.0;
+    load_fields(ci, cj, ck, f0, f1);
+
+    // incoming batch descriptor (warp-uniform) and its particle registers
+    unsigned long long lv_acc = 0;
+    int in_state = 0;            // 0 none, 1 belongs to the current cell, 2 to the next cell, 3 next cell looked empty
+    int in_s = 0, in_nb = 0;
+    uint32_t in_p0 = 0;
+    ParticleRegs in;
+    in.x = in.y = in.z = in.u = in.v = in.w = in.q = 0.0;
+    {
+        const unsigned ne = __ballot_sync(0xffffffffu, lane < nsp && sb < se);
+        if (ne) {
+            in_s = __ffs(ne) - 1;
+            in_p0 = __shfl_sync(0xffffffffu, sb, in_s);
+            in_nb = (int)min(32u, __shfl_sync(0xffffffffu, se, in_s) - in_p0);
+            in_state = 1;
+            load_batch(a.sp[in_s], in_p0, in_nb, lane, in);
+        }
+    }
+
+    // accumulators: C[mt][nt], class 8 mt + fr, columns 8 nt + 2 fk + {0,1}
+    double2 acc[4][2];
+#pragma unroll
+    for (int mt = 0; mt < 4; ++mt) { acc[mt][0] = make_double2(0.0, 0.0); acc[mt][1] = make_double2(0.0, 0.0); }
+
+    for (uint32_t c = c_lo; c < c_hi; ++c) {
+        // ---- cell prologue: publish this cell's corner fields, prefetch the next cell's ----
+        fld[lane] = f0;
+        if (lane < FLD_DOUBLES - 32) fld[lane + 32] = f1;
+        const bool has_next = c + 1 < c_hi;
+        int nk = ck + 1, nj = cj, ni = ci;
+        if (nk == g.nz) { nk = 0; nj = cj + 1; if (nj == g.ny) { nj = 0; ni = ci + 1; } }
+        if (has_next) load_fields(ni, nj, nk, f0, f1);
+        __syncwarp();
+        const double dci = (double)ci, dcj = (double)cj, dck = (double)ck;
+        const unsigned ne_cur = __ballot_sync(0xffffffffu, lane < nsp && sb < se);
+        unsigned my_leavers = 0;
+
+        while (in_state == 1) {
+            // ---- take the incoming batch ----
+            const int s = in_s, nb = in_nb;
+            const uint32_t p0 = in_p0;
+            const ParticleRegs cur = in;
+            const SpeciesDev& sp = a.sp[s];
+
+            // ---- descriptor of the batch after this one ----
+            {
+                const uint32_t e = __shfl_sync(0xffffffffu, se, s);
+                const unsigned later = ne_cur & ~((2u << s) - 1u);
+                if (p0 + 32 < e) {
+                    in_p0 = p0 + 32;
+                    in_nb = (int)min(32u, e - in_p0);
+                } else if (later) {
+                    in_s = __ffs(later) - 1;
+                    in_p0 = __shfl_sync(0xffffffffu, sb, in_s);
+                    in_nb = (int)min(32u, __shfl_sync(0xffffffffu, se, in_s) - in_p0);
+                } else {
+                    const unsigned ne_next = __ballot_sync(0xffffffffu, has_next && lane < nsp && se < sn);
+                    if (ne_next) {
+                        in_s = __ffs(ne_next) - 1;
+                        in_p0 = __shfl_sync(0xffffffffu, se, in_s);
+                        in_nb = (int)min(32u, __shfl_sync(0xffffffffu, sn, in_s) - in_p0);
+                        in_state = 2;
+                    } else {
+                        in_state = has_next ? 3 : 0;   // 3: the next cell is empty, look again there
+                    }
+                }
+            }
+
+            // ---- phase 1: lane = particle ----
+            const bool stray = phase1(g, sp, cur, lane < nb, p0 + lane, sp.beta, dt, dci, dcj, dck, fld, stcol, my_leavers);
+            // global loads of the next batch fly during phase 2
+            if (in_state == 1 || in_state == 2) load_batch(a.sp[in_s], in_p0, in_nb, lane, in);
+            const unsigned smask = __ballot_sync(0xffffffffu, stray);
+            if (smask) {
+                uint32_t base = 0;
+                if (lane == 0) base = atomicAdd(sp.stray_count, (uint32_t)__popc(smask));
+                base = __shfl_sync(0xffffffffu, base, 0);
+                if (stray) sp.stray_list[base + __popc(smask & ((1u << lane) - 1u))] = p0 + lane;
+            }
+            __syncwarp();
+
+            // ---- phase 2: C += c^T b over the batch, four particles per DMMA (columns >= nb hold c = 0) ----
+            if (nb > 28) {
+#pragma unroll
+                for (int gq = 0; gq < 8; ++gq) {
+                    const double* f = frag + gq * 4;
+                    const double b0 = f[ROW_B * ST_PITCH], b1 = f[(ROW_B + 8) * ST_PITCH];
+#pragma unroll
+                    for (int mt = 0; mt < 4; ++mt) {
+                        const double av = f[(ROW_C + 8 * mt) * ST_PITCH];
+                        dmma_m8n8k4(acc[mt][0], av, b0);
+                        dmma_m8n8k4(acc[mt][1], av, b1);
+                    }
+                }
+            } else {
+                const int ng = (nb + 3) >> 2;
+#pragma unroll 1
+                for (int gq = 0; gq < ng; ++gq) {
+                    const double* f = frag + gq * 4;
+                    const double b0 = f[ROW_B * ST_PITCH], b1 = f[(ROW_B + 8) * ST_PITCH];
+#pragma unroll
+                    for (int mt = 0; mt < 4; ++mt) {
+                        const double av = f[(ROW_C + 8 * mt) * ST_PITCH];
+                        dmma_m8n8k4(acc[mt][0], av, b0);
+                        dmma_m8n8k4(acc[mt][1], av, b1);
+                    }
+                }
+            }
+            __syncwarp();
+
+            // ---- end of a species in this cell: fold its rho/Jhat class sums to the 8 corners, one store ----
+            if (in_state != 1 || in_s != s) {
+                // lanes fk = 0: (rho, Jx), fk = 1: (Jy, Jz) of class 8 mt + fr -> T[class][4] over staging rows 0..2
+                if (fk < 2) {
+#pragma unroll
+                    for (int mt = 0; mt < 4; ++mt) {
+                        const int cls = 8 * mt + fr;
+                        if (cls < 27) *reinterpret_cast<double2*>(stg + cls * 4 + 2 * fk) = acc[mt][1];
+                        acc[mt][1] = make_double2(0.0, 0.0);
+                    }
+                }
+                __syncwarp();
+                {
+                    // lane = (corner, component): W_N = sum of the 8 classes pairing N with any N' of the cell
+                    const int cn = lane >> 2, comp = lane & 3;
+                    const double* t = stg + (((cn >> 2) & 1) * 9 + ((cn >> 1) & 1) * 3 + (cn & 1)) * 4 + comp;
+                    const double sum = ((t[0] + t[4]) + (t[12] + t[16])) + ((t[36] + t[40]) + (t[48] + t[52]));
+                    sp.AJ[(size_t)c * AJ_PER_CELL + lane] = sum;
+                }
+                my_leavers = __reduce_add_sync(0xffffffffu, my_leavers);
+                if (lane == s) lv_acc += my_leavers;     // lane s keeps the warp's count for species s
+                my_leavers = 0;
+                __syncwarp();
+            }
+        }
+
+        // species without particles in this cell still own an AJ block: zeros
+        {
+            unsigned empty = ~ne_cur & ((nsp >= 32) ? 0xffffffffu : ((1u << nsp) - 1u));
+            while (empty) {
+                const int s = __ffs(empty) - 1;
+                empty &= empty - 1;
+                a.sp[s].AJ[(size_t)c * AJ_PER_CELL + lane] = 0.0;
+            }
+        }
+
+        // ---- mass-matrix classes of this cell: straight from the fragments, 16-byte coalesced stores ----
+        {
+            double* dst = a.AM + (size_t)c * AM_PER_CELL;
+#pragma unroll
+            for (int mt = 0; mt < 4; ++mt) {
+                const int cls = 8 * mt + fr;
+                if (cls < 27) {
+                    *reinterpret_cast<double2*>(dst + mt * 64 + fr * 8 + 2 * fk) = acc[mt][0];
+                    if (fk == 2) dst[AM_A8 + cls] = acc[mt][1].x;
+                }
+                acc[mt][0] = make_double2(0.0, 0.0);
+                acc[mt][1] = make_double2(0.0, 0.0);
+            }
+        }
+
+        // ---- advance to the next cell ----
+        if (lane < nsp) {
+            sb = se; se = sn;
+            if (c + 2 < c_hi) sn = __ldg(my_start + c + 3);
+        }
+        ci = ni; cj = nj; ck = nk;
+        if (in_state == 2) {
+            in_state = 1;
+        } else if (has_next) {
+            // nothing was prefetched for the cell just entered (it looked empty, or the previous cell had
+            // no batch to prefetch from): look for its first batch now
+            const unsigned ne = __ballot_sync(0xffffffffu, lane < nsp && sb < se);
+            in_state = 0;
+            if (ne) {
+                in_s = __ffs(ne) - 1;
+                in_p0 = __shfl_sync(0xffffffffu, sb, in_s);
+                in_nb = (int)min(32u, __shfl_sync(0xffffffffu, se, in_s) - in_p0);
+                in_state = 1;
+                load_batch(a.sp[in_s], in_p0, in_nb, lane, in);
+            }
+        }
+    }
+    if (lane < nsp && lv_acc) atomicAdd(a.sp[lane].leavers, lv_acc);
+}
