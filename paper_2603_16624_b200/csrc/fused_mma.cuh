@@ -39,8 +39,13 @@
 
 constexpr int ST_PITCH = 36;     // doubles per staging row: 32 particles + 4 (pitch = 4 mod 16: LDS.64 conflict-free)
 constexpr int ROW_C = 0;         // rows 0..26: the 27 classes, class = kx*9 + ky*3 + kz
-constexpr int ROW_B = 27;        // rows 27..34: beta*alpha[0..7]; 35: 1; 36..38: alpha v^n; 39: beta*alpha[8]; 40..42: zero
-constexpr int ST_ROWS = 43;      // A tile 3 reads rows 24..31 (27..31 = finite junk for the 5 unused classes)
+constexpr int ROW_WQ = 27;       // rows 27..34: q/V * W[8], corner = a*4 + b*2 + c (also the junk rows 27..31 of A tile 3)
+constexpr int ROW_BA = 35;       // rows 35..42: beta*alpha[0..7]
+constexpr int ROW_A8 = 43;       // row 43: beta*alpha[8]
+constexpr int ROW_ONE = 44;      // row 44: 1 (constant);  rows 45..47: alpha v^n
+constexpr int ROW_VH = 45;
+constexpr int ROW_BJ = 40;       // B tile of the rho/Jhat contraction: rows 40..47, useful columns 4..7 = (1, vhat)
+constexpr int ST_ROWS = 48;
 constexpr int FLD_DOUBLES = 48;  // 8 corners x (Ex,Ey,Ez,Bx,By,Bz)
 constexpr int WARP_SMEM_DOUBLES = ST_ROWS * ST_PITCH + FLD_DOUBLES;
 constexpr int AM_PER_CELL = 288; // [4 m-tiles][8 classes][8 alpha entries] + [32 classes] alpha[8]
@@ -134,9 +139,11 @@ __device__ __forceinline__ bool phase1(const Geom& g, const SpeciesDev& sp, cons
     const double q = inside ? r.q : 0.0;
     const double wx0 = 1.0 - xi, wy0 = 1.0 - eta, wz0 = 1.0 - zeta;
     double Ex = 0, Ey = 0, Ez = 0, Bx = 0, By = 0, Bz = 0;
+    double W[8];
     {
         const double w00 = wx0 * wy0, w01 = wx0 * eta, w10 = xi * wy0, w11 = xi * eta;
-        const double W[8] = {w00 * wz0, w00 * zeta, w01 * wz0, w01 * zeta, w10 * wz0, w10 * zeta, w11 * wz0, w11 * zeta};
+        W[0] = w00 * wz0; W[1] = w00 * zeta; W[2] = w01 * wz0; W[3] = w01 * zeta;
+        W[4] = w10 * wz0; W[5] = w10 * zeta; W[6] = w11 * wz0; W[7] = w11 * zeta;
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
             const double2 f0 = *reinterpret_cast<const double2*>(fld + k * 6);
@@ -153,17 +160,23 @@ __device__ __forceinline__ bool phase1(const Geom& g, const SpeciesDev& sp, cons
     const double a00 = fma(bx, sx, invD), a01 = fma(bx, sy, sz), a02 = fma(bx, sz, -sy);
     const double a10 = fma(by, sx, -sz), a11 = fma(by, sy, invD), a12 = fma(by, sz, sx);
     const double a20 = fma(bz, sx, sy), a21 = fma(bz, sy, -sx), a22 = fma(bz, sz, invD);
-    // deposit factors (pre-push x and v, L49): B operand of the contraction
-    double* sb = st + ROW_B * ST_PITCH;
-    sb[0 * ST_PITCH] = beta * a00; sb[1 * ST_PITCH] = beta * a01; sb[2 * ST_PITCH] = beta * a02;
-    sb[3 * ST_PITCH] = beta * a10; sb[4 * ST_PITCH] = beta * a11; sb[5 * ST_PITCH] = beta * a12;
-    sb[6 * ST_PITCH] = beta * a20; sb[7 * ST_PITCH] = beta * a21; sb[12 * ST_PITCH] = beta * a22;
-    sb[9 * ST_PITCH] = a00 * vx + a01 * vy + a02 * vz;
-    sb[10 * ST_PITCH] = a10 * vx + a11 * vy + a12 * vz;
-    sb[11 * ST_PITCH] = a20 * vx + a21 * vy + a22 * vz;
+    // deposit factors (pre-push x and v, L49): operands of the contractions, one column per particle
     {
-        // A operand, 27 classes: q/V * px[kx] * py[ky] * pz[kz]
+        double* sb = st + ROW_BA * ST_PITCH;
+        sb[0 * ST_PITCH] = beta * a00; sb[1 * ST_PITCH] = beta * a01; sb[2 * ST_PITCH] = beta * a02;
+        sb[3 * ST_PITCH] = beta * a10; sb[4 * ST_PITCH] = beta * a11; sb[5 * ST_PITCH] = beta * a12;
+        sb[6 * ST_PITCH] = beta * a20; sb[7 * ST_PITCH] = beta * a21; sb[8 * ST_PITCH] = beta * a22;
+        double* sv = st + ROW_VH * ST_PITCH;
+        sv[0 * ST_PITCH] = a00 * vx + a01 * vy + a02 * vz;
+        sv[1 * ST_PITCH] = a10 * vx + a11 * vy + a12 * vz;
+        sv[2 * ST_PITCH] = a20 * vx + a21 * vy + a22 * vz;
+    }
+    {
         const double qV = q * g.invV;
+        double* sw = st + ROW_WQ * ST_PITCH;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) sw[k * ST_PITCH] = qV * W[k];
+        // 27 classes: q/V * px[kx] * py[ky] * pz[kz]
         const double qx0 = qV * wx0, qx1 = qV * xi;
         const double px[3] = {qx0 * wx0, qx0 * xi, qx1 * xi};
         const double py[3] = {wy0 * wy0, wy0 * eta, eta * eta};
@@ -206,7 +219,7 @@ k_fused_push_moments(const __grid_constant__ FusedArgs a)
     double* fld = stg + ST_ROWS * ST_PITCH;
     for (int t = lane; t < WARP_SMEM_DOUBLES; t += 32) stg[t] = 0.0;
     __syncwarp();
-    for (int t = lane; t < ST_PITCH; t += 32) stg[(ROW_B + 8) * ST_PITCH + t] = 1.0;   // the rho column of b
+    for (int t = lane; t < ST_PITCH; t += 32) stg[ROW_ONE * ST_PITCH + t] = 1.0;   // the rho column of the rho/Jhat B tile
     __syncwarp();
 
     const Geom& g = a.g;
@@ -275,10 +288,14 @@ k_fused_push_moments(const __grid_constant__ FusedArgs a)
         }
     }
 
-    // accumulators: C[mt][nt], class 8 mt + fr, columns 8 nt + 2 fk + {0,1}
-    double2 acc[4][2];
+    // accumulators (lane = row fr of a tile, particle fk of a group of four):
+    //   accM[mt]  C tile of sum_p c[8 mt + fr] * beta alpha[2 fk + {0,1}]            (DMMA)
+    //   acc8[mt]  this lane's share (particles = fk mod 4) of sum_p c[8 mt + fr] * beta alpha[8]   (DFMA on the A fragment)
+    //   accJ      C tile of sum_p q/V W[fr] * (.., .., .., .., 1, vhat): fk = 2 holds (rho, Jx), fk = 3 (Jy, Jz)
+    double2 accM[4], accJ = make_double2(0.0, 0.0);
+    double acc8[4];
 #pragma unroll
-    for (int mt = 0; mt < 4; ++mt) { acc[mt][0] = make_double2(0.0, 0.0); acc[mt][1] = make_double2(0.0, 0.0); }
+    for (int mt = 0; mt < 4; ++mt) { accM[mt] = make_double2(0.0, 0.0); acc8[mt] = 0.0; }
 
     for (uint32_t c = c_lo; c < c_hi; ++c) {
         // ---- cell prologue: publish this cell's corner fields, prefetch the next cell's ----
@@ -337,58 +354,36 @@ k_fused_push_moments(const __grid_constant__ FusedArgs a)
             }
             __syncwarp();
 
-            // ---- phase 2: C += c^T b over the batch, four particles per DMMA (columns >= nb hold c = 0) ----
-            if (nb > 28) {
-#pragma unroll
-                for (int gq = 0; gq < 8; ++gq) {
-                    const double* f = frag + gq * 4;
-                    const double b0 = f[ROW_B * ST_PITCH], b1 = f[(ROW_B + 8) * ST_PITCH];
-#pragma unroll
-                    for (int mt = 0; mt < 4; ++mt) {
-                        const double av = f[(ROW_C + 8 * mt) * ST_PITCH];
-                        dmma_m8n8k4(acc[mt][0], av, b0);
-                        dmma_m8n8k4(acc[mt][1], av, b1);
-                    }
-                }
-            } else {
-                const int ng = (nb + 3) >> 2;
+            // ---- phase 2: contractions over the batch, four particles per step (columns >= nb hold c = 0, Wq = 0) ----
+            {
+                const int ng = nb > 28 ? 8 : (nb + 3) >> 2;
 #pragma unroll 1
-                for (int gq = 0; gq < ng; ++gq) {
-                    const double* f = frag + gq * 4;
-                    const double b0 = f[ROW_B * ST_PITCH], b1 = f[(ROW_B + 8) * ST_PITCH];
+                for (int gq = 0; gq < ng; gq += 2) {
 #pragma unroll
-                    for (int mt = 0; mt < 4; ++mt) {
-                        const double av = f[(ROW_C + 8 * mt) * ST_PITCH];
-                        dmma_m8n8k4(acc[mt][0], av, b0);
-                        dmma_m8n8k4(acc[mt][1], av, b1);
+                    for (int h = 0; h < 2; ++h) {
+                        // ng odd: the extra group reads valid columns whose c and Wq are zero
+                        const double* f = frag + (gq + h) * 4;
+                        const double b0 = f[ROW_BA * ST_PITCH], a8 = f[(ROW_A8 - fr) * ST_PITCH];
+                        const double wq = f[ROW_WQ * ST_PITCH], bj = f[ROW_BJ * ST_PITCH];
+#pragma unroll
+                        for (int mt = 0; mt < 4; ++mt) {
+                            const double av = f[(ROW_C + 8 * mt) * ST_PITCH];
+                            dmma_m8n8k4(accM[mt], av, b0);
+                            acc8[mt] = fma(av, a8, acc8[mt]);
+                        }
+                        dmma_m8n8k4(accJ, wq, bj);
                     }
                 }
             }
             __syncwarp();
 
-            // ---- end of a species in this cell: fold its rho/Jhat class sums to the 8 corners, one store ----
+            // ---- end of a species in this cell: its rho/Jhat corner sums, straight from the fragment ----
             if (in_state != 1 || in_s != s) {
-                // lanes fk = 0: (rho, Jx), fk = 1: (Jy, Jz) of class 8 mt + fr -> T[class][4] over staging rows 0..2
-                if (fk < 2) {
-#pragma unroll
-                    for (int mt = 0; mt < 4; ++mt) {
-                        const int cls = 8 * mt + fr;
-                        if (cls < 27) *reinterpret_cast<double2*>(stg + cls * 4 + 2 * fk) = acc[mt][1];
-                        acc[mt][1] = make_double2(0.0, 0.0);
-                    }
-                }
-                __syncwarp();
-                {
-                    // lane = (corner, component): W_N = sum of the 8 classes pairing N with any N' of the cell
-                    const int cn = lane >> 2, comp = lane & 3;
-                    const double* t = stg + (((cn >> 2) & 1) * 9 + ((cn >> 1) & 1) * 3 + (cn & 1)) * 4 + comp;
-                    const double sum = ((t[0] + t[4]) + (t[12] + t[16])) + ((t[36] + t[40]) + (t[48] + t[52]));
-                    sp.AJ[(size_t)c * AJ_PER_CELL + lane] = sum;
-                }
+                if (fk >= 2) *reinterpret_cast<double2*>(sp.AJ + (size_t)c * AJ_PER_CELL + fr * 4 + 2 * (fk - 2)) = accJ;
+                accJ = make_double2(0.0, 0.0);
                 my_leavers = __reduce_add_sync(0xffffffffu, my_leavers);
                 if (lane == s) lv_acc += my_leavers;     // lane s keeps the warp's count for species s
                 my_leavers = 0;
-                __syncwarp();
             }
         }
 
@@ -408,12 +403,15 @@ k_fused_push_moments(const __grid_constant__ FusedArgs a)
 #pragma unroll
             for (int mt = 0; mt < 4; ++mt) {
                 const int cls = 8 * mt + fr;
+                double s8 = acc8[mt];
+                s8 += shfl_xor_f64(s8, 1);
+                s8 += shfl_xor_f64(s8, 2);
                 if (cls < 27) {
-                    *reinterpret_cast<double2*>(dst + mt * 64 + fr * 8 + 2 * fk) = acc[mt][0];
-                    if (fk == 2) dst[AM_A8 + cls] = acc[mt][1].x;
+                    *reinterpret_cast<double2*>(dst + mt * 64 + fr * 8 + 2 * fk) = accM[mt];
+                    if (fk == 0) dst[AM_A8 + cls] = s8;
                 }
-                acc[mt][0] = make_double2(0.0, 0.0);
-                acc[mt][1] = make_double2(0.0, 0.0);
+                accM[mt] = make_double2(0.0, 0.0);
+                acc8[mt] = 0.0;
             }
         }
 
