@@ -518,6 +518,7 @@ static int push_and_moments_impl(ecsim_ctx* c, int n_list, const int* list, cons
         d.start = w.start + (size_t)s * (cells + 1);
         d.x = sp.x; d.y = sp.y; d.z = sp.z; d.u = sp.u; d.v = sp.v; d.w = sp.w; d.q = sp.q;
         d.beta = sp.qom * dt / 2.0;
+        d.n = (uint32_t)sp.n;
         d.AJ = w.AJ + (size_t)s * cells * AJ_PER_CELL;
         d.stray_list = w.stray_list + (size_t)s * (size_t)w.n_max;
         d.stray_count = w.stray_count + s;

@@ -10,15 +10,14 @@
 // (Eq. 3 summed over the particles of every cell that holds both N and N').
 //
 // k_expand_M: one CTA walks EXPAND_Z consecutive nodes of one (i,j) column; thread t < 243 owns one
-// element (o, ij).  Threads are ordered by the LENGTH of their term list (8, 4, 2, 1) so that a warp's
-// loop count is uniform and short, every load of a node is issued before the first use (straight-line
-// code per term count: the memory-level parallelism the first version lacked, profiles/r01a), and two
-// nodes are in flight per iteration.
+// element (o, ij).  Threads are ordered by the SHAPE of their term list ((x-y terms) x (z terms)) so that
+// a warp's load count is uniform and short, and every load of a node is issued before the first use
+// (straight-line code per shape: the memory-level parallelism the first version lacked, profiles/r01a).
 #pragma once
 #include "common.cuh"
 #include "fused_mma.cuh"
 
-constexpr int EXPAND_Z = 16;
+constexpr int EXPAND_Z = 32;
 
 struct ExpandArgs {
     Geom g;
@@ -27,58 +26,45 @@ struct ExpandArgs {
     int accumulate;
 };
 
-// neighbour slots ordered by term count: o = 13 (8 terms); the 6 face slots (4); the 12 edge slots (2);
-// the 8 corner slots (1)
+// neighbour slots ordered by (x-y terms, z terms) = (4,2) | (4,1) | (2,2) | (2,1) | (1,2) | (1,1)
 __device__ __constant__ unsigned char EXPAND_ORDER[27] = {
     13,
-    4, 10, 12, 14, 16, 22,
-    1, 3, 5, 7, 9, 11, 15, 17, 19, 21, 23, 25,
+    12, 14,
+    4, 10, 16, 22,
+    3, 5, 9, 11, 15, 17, 21, 23,
+    1, 7, 19, 25,
     0, 2, 6, 8, 18, 20, 24, 26};
 
-// offset, in doubles inside a cell's AM block, of (class, ij)
-__device__ __forceinline__ int am_elem(int cls, int ij)
-{
-    return ij < 8 ? ((cls >> 3) * 64 + (cls & 7) * 8 + ij) : (AM_A8 + cls);
-}
-
-template <int NT>
-__device__ __forceinline__ void expand_nodes(const ExpandArgs& a, const size_t (&off)[8], unsigned zbits, int T,
-                                             int k0, int k1, double* __restrict__ dst0)
+// Offset, in doubles inside a cell's AM block, of (class, ij): 8*class + ij for ij < 8, AM_A8 + class for
+// ij = 8 -- additive in the per-axis parts of class = 9 clx + 3 cly + clz.
+template <int NXY, int NTZ>
+__device__ __forceinline__ void expand_nodes(const ExpandArgs& a, const double* const (&col)[4], int ezA, int ezB,
+                                             bool zA_is_prev, int nxy, int ntz, int k0, int k1,
+                                             double* __restrict__ dst0)
 {
     const int nz = a.g.nz;
-    int k = k0;
-    for (; k + 1 < k1; k += 2) {
-        const size_t zA0 = (size_t)k * AM_PER_CELL, zB0 = (size_t)(k ? k - 1 : nz - 1) * AM_PER_CELL;
-        const size_t zA1 = (size_t)(k + 1) * AM_PER_CELL, zB1 = zA0;
-        double v0[NT], v1[NT];
+#pragma unroll 2
+    for (int k = k0; k < k1; ++k) {
+        // z terms: A = first entry of the z list, B = second (cell k-1, class 2) when dz = 0
+        const int km1 = k ? k - 1 : nz - 1;
+        const int zA = (zA_is_prev ? km1 : k) * AM_PER_CELL + ezA, zB = km1 * AM_PER_CELL + ezB;
+        double v[NXY][NTZ];
 #pragma unroll
-        for (int t = 0; t < NT; ++t) {
-            v0[t] = __ldg(a.AM + off[t] + (((zbits >> t) & 1u) ? zB0 : zA0));
-            v1[t] = __ldg(a.AM + off[t] + (((zbits >> t) & 1u) ? zB1 : zA1));
+        for (int t = 0; t < NXY; ++t) {
+            v[t][0] = __ldg(col[t] + zA);
+            if (NTZ == 2) v[t][1] = __ldg(col[t] + zB);
         }
-        double s0 = 0.0, s1 = 0.0;
-        if (a.accumulate) { s0 = dst0[(size_t)k * 243]; s1 = dst0[(size_t)(k + 1) * 243]; }
+        double s = a.accumulate ? dst0[(size_t)k * 243] : 0.0;
 #pragma unroll
-        for (int t = 0; t < NT; ++t) {
-            s0 += t < T ? v0[t] : 0.0;
-            s1 += t < T ? v1[t] : 0.0;
+        for (int t = 0; t < NXY; ++t) {
+            s += t < nxy ? v[t][0] : 0.0;
+            if (NTZ == 2) s += (t < nxy && ntz == 2) ? v[t][1] : 0.0;
         }
-        dst0[(size_t)k * 243] = s0;
-        dst0[(size_t)(k + 1) * 243] = s1;
-    }
-    if (k < k1) {
-        const size_t zA0 = (size_t)k * AM_PER_CELL, zB0 = (size_t)(k ? k - 1 : nz - 1) * AM_PER_CELL;
-        double v0[NT];
-#pragma unroll
-        for (int t = 0; t < NT; ++t) v0[t] = __ldg(a.AM + off[t] + (((zbits >> t) & 1u) ? zB0 : zA0));
-        double s0 = a.accumulate ? dst0[(size_t)k * 243] : 0.0;
-#pragma unroll
-        for (int t = 0; t < NT; ++t) s0 += t < T ? v0[t] : 0.0;
-        dst0[(size_t)k * 243] = s0;
+        dst0[(size_t)k * 243] = s;
     }
 }
 
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 4)
 k_expand_M(const __grid_constant__ ExpandArgs a)
 {
     const int t = threadIdx.x;
@@ -91,33 +77,39 @@ k_expand_M(const __grid_constant__ ExpandArgs a)
     const int j = (int)((blockIdx.x / (unsigned)zchunks) % (unsigned)g.ny);
     const int i = (int)(blockIdx.x / ((unsigned)zchunks * (unsigned)g.ny));
     const int im1 = i ? i - 1 : g.nx - 1, jm1 = j ? j - 1 : g.ny - 1;
+    const int ebase = ij < 8 ? ij : AM_A8, emul = ij < 8 ? 8 : 1;
 
-    // per-axis term lists: (cell index or z selector, class)
+    // x and y term lists: (cell index, class); d = 0: (own, 0), (previous, 2); d = +1: (own, 1); d = -1: (previous, 1)
     const int ntx = dx == 0 ? 2 : 1, nty = dy == 0 ? 2 : 1, ntz = dz == 0 ? 2 : 1;
-    const int cix[2] = {dx >= 0 ? i : im1, im1}, clx[2] = {dx == 0 ? 0 : 1, 2};
-    const int cjy[2] = {dy >= 0 ? j : jm1, jm1}, cly[2] = {dy == 0 ? 0 : 1, 2};
-    const int zsel[2] = {dz >= 0 ? 0 : 1, 1}, clz[2] = {dz == 0 ? 0 : 1, 2};   // zsel 1 = cell k-1
-    const int T = ntx * nty * ntz;
-    size_t off[8];
-    unsigned zbits = 0;
+    const int nxy = ntx * nty;
+    const double* col[4];
 #pragma unroll
-    for (int e = 0; e < 8; ++e) {
-        // term e < T in mixed radix (ntx, nty, ntz); e >= T repeats term 0 (its value is not added)
-        const int ee = e < T ? e : 0;
-        const int tz = ee % ntz, ty = (ee / ntz) % nty, tx = ee / (ntz * nty);
-        off[e] = ((size_t)cix[tx] * g.ny + cjy[ty]) * g.nz * AM_PER_CELL +
-                 (size_t)am_elem(clx[tx] * 9 + cly[ty] * 3 + clz[tz], ij);
-        zbits |= (unsigned)zsel[tz] << e;
+    for (int e = 0; e < 4; ++e) {
+        const int ee = e < nxy ? e : 0;                 // e >= nxy repeats term 0 (its value is not added)
+        const int ty = ee % nty, tx = ee / nty;
+        const int ci = tx == 0 ? (dx >= 0 ? i : im1) : im1, cx = tx == 0 ? (dx == 0 ? 0 : 1) : 2;
+        const int cj = ty == 0 ? (dy >= 0 ? j : jm1) : jm1, cy = ty == 0 ? (dy == 0 ? 0 : 1) : 2;
+        col[e] = a.AM + ((size_t)ci * g.ny + cj) * g.nz * AM_PER_CELL + (ebase + emul * (9 * cx + 3 * cy));
     }
+    // z list: dz = 0: (cell k, class 0), (cell k-1, class 2); dz = +1: (cell k, class 1); dz = -1: (cell k-1, class 1)
+    const int ezA = emul * (dz == 0 ? 0 : 1), ezB = emul * 2;
+    const bool zA_is_prev = dz < 0;
+
     const int k0 = zc * EXPAND_Z;
     const int k1 = min(k0 + EXPAND_Z, g.nz);
     double* dst0 = a.M + ((size_t)i * g.ny + j) * g.nz * 243 + (size_t)(o * 9 + ij);
-    // longest term list in the warp (the thread order makes it 8, 4, 2, 2, 2, 2, 1, 1 for warps 0..7)
-    const int Tw = __reduce_max_sync(__activemask(), T);
-    if (Tw == 8) expand_nodes<8>(a, off, zbits, T, k0, k1, dst0);
-    else if (Tw == 4) expand_nodes<4>(a, off, zbits, T, k0, k1, dst0);
-    else if (Tw == 2) expand_nodes<2>(a, off, zbits, T, k0, k1, dst0);
-    else expand_nodes<1>(a, off, zbits, T, k0, k1, dst0);
+    // longest lists in the warp: warps 0..7 see (4,2), (2,2), (2,1), (2,1), (2,2), (1,2), (1,1), (1,1)
+    const unsigned am = __activemask();
+    const int wxy = __reduce_max_sync(am, nxy), wz = __reduce_max_sync(am, ntz);
+    if (wz == 2) {
+        if (wxy == 4) expand_nodes<4, 2>(a, col, ezA, ezB, zA_is_prev, nxy, ntz, k0, k1, dst0);
+        else if (wxy == 2) expand_nodes<2, 2>(a, col, ezA, ezB, zA_is_prev, nxy, ntz, k0, k1, dst0);
+        else expand_nodes<1, 2>(a, col, ezA, ezB, zA_is_prev, nxy, ntz, k0, k1, dst0);
+    } else {
+        if (wxy == 4) expand_nodes<4, 1>(a, col, ezA, ezB, zA_is_prev, nxy, ntz, k0, k1, dst0);
+        else if (wxy == 2) expand_nodes<2, 1>(a, col, ezA, ezB, zA_is_prev, nxy, ntz, k0, k1, dst0);
+        else expand_nodes<1, 1>(a, col, ezA, ezB, zA_is_prev, nxy, ntz, k0, k1, dst0);
+    }
 }
 
 struct ExpandJArgs {

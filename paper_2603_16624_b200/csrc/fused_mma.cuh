@@ -58,6 +58,7 @@ struct SpeciesDev {
     double *x, *y, *z, *u, *v, *w;
     const double* q;
     double beta;             // q dt/(2m) (L55)
+    uint32_t n;              // particles of the species
     double* AJ;              // [cells][8][4]: rho, Jx, Jy, Jz per corner
     uint32_t* stray_list;
     uint32_t* stray_count;
@@ -95,6 +96,18 @@ __device__ __forceinline__ void dmma_m8n8k4(double2& d, double a, double b)
                  : "+d"(d.x), "+d"(d.y) : "d"(a), "d"(b));
 }
 
+// 1/d for finite d >= 1 (D = 1 + |b|^2 of Eq. 2): hardware seed (~20 bits) and two Newton steps; no
+// subnormal / infinity / zero path is needed for this range.  Error <= 1 ulp.
+__device__ __forceinline__ double rcp_ge1(double d)
+{
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(d));
+    double e = fma(-d, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-d, r, 1.0);
+    return fma(r, e, r);
+}
+
 // First cell of warp w's range: smallest c with  CELL_WEIGHT*c + sum_s start_s[c] >= w/W of the total.
 __device__ __forceinline__ uint32_t range_bound(const FusedArgs& a, uint32_t w, uint32_t W)
 {
@@ -113,16 +126,6 @@ __device__ __forceinline__ uint32_t range_bound(const FusedArgs& a, uint32_t w, 
 }
 
 struct ParticleRegs { double x, y, z, u, v, w, q; };
-
-__device__ __forceinline__ void load_batch(const SpeciesDev& sp, uint32_t p0, int nb, int lane, ParticleRegs& r)
-{
-    if (lane < nb) {
-        const uint32_t p = p0 + lane;
-        r.x = sp.x[p]; r.y = sp.y[p]; r.z = sp.z[p];
-        r.u = sp.u[p]; r.v = sp.v[p]; r.w = sp.w[p];
-        r.q = __ldg(sp.q + p);
-    }
-}
 
 // Phase 1 for one lane: returns true if the lane holds a stray.  `st` = staging tile + lane (the
 // lane's column), `fld` = the cell's corner fields, (dci,dcj,dck) = the cell's integer coordinates.
@@ -155,7 +158,7 @@ __device__ __forceinline__ bool phase1(const Geom& g, const SpeciesDev& sp, cons
     }
     // alpha_p, Eq. (2): (I x B) v = B x v, b = beta B_p;  alpha = (I + [b]x)^-1
     const double bx = beta * Bx, by = beta * By, bz = beta * Bz;
-    const double invD = 1.0 / (1.0 + (bx * bx + by * by + bz * bz));
+    const double invD = rcp_ge1(1.0 + (bx * bx + by * by + bz * bz));
     const double sx = invD * bx, sy = invD * by, sz = invD * bz;
     const double a00 = fma(bx, sx, invD), a01 = fma(bx, sy, sz), a02 = fma(bx, sz, -sy);
     const double a10 = fma(by, sx, -sz), a11 = fma(by, sy, invD), a12 = fma(by, sz, sx);
@@ -215,6 +218,7 @@ k_fused_push_moments(const __grid_constant__ FusedArgs a)
 {
     extern __shared__ __align__(16) double smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
     double* stg = smem + (size_t)warp * WARP_SMEM_DOUBLES;
     double* fld = stg + ST_ROWS * ST_PITCH;
     for (int t = lane; t < WARP_SMEM_DOUBLES; t += 32) stg[t] = 0.0;
@@ -267,8 +271,10 @@ k_fused_push_moments(const __grid_constant__ FusedArgs a)
         se = __ldg(my_start + c_lo + 1);
         if (c_lo + 1 < c_hi) sn = __ldg(my_start + c_lo + 2);
     }
+    // corner fields of the NEXT cell are requested while the last batch of a cell is in phase 2, so that
+    // their registers are not live across a phase 1 (fld_ready: warp-uniform)
     double f0 = 0.0, f1 = 0.0;
-    load_fields(ci, cj, ck, f0, f1);
+    bool fld_ready = false;
 
     // incoming batch descriptor (warp-uniform) and its particle registers
     unsigned long long lv_acc = 0;
@@ -298,13 +304,14 @@ k_fused_push_moments(const __grid_constant__ FusedArgs a)
     for (int mt = 0; mt < 4; ++mt) { accM[mt] = make_double2(0.0, 0.0); acc8[mt] = 0.0; }
 
     for (uint32_t c = c_lo; c < c_hi; ++c) {
-        // ---- cell prologue: publish this cell's corner fields, prefetch the next cell's ----
+        // ---- cell prologue: publish this cell's corner fields ----
+        if (!fld_ready) load_fields(ci, cj, ck, f0, f1);     // first cell of the range, or after an empty cell
         fld[lane] = f0;
         if (lane < FLD_DOUBLES - 32) fld[lane + 32] = f1;
+        fld_ready = false;
         const bool has_next = c + 1 < c_hi;
         int nk = ck + 1, nj = cj, ni = ci;
         if (nk == g.nz) { nk = 0; nj = cj + 1; if (nj == g.ny) { nj = 0; ni = ci + 1; } }
-        if (has_next) load_fields(ni, nj, nk, f0, f1);
         __syncwarp();
         const double dci = (double)ci, dcj = (double)cj, dck = (double)ck;
         const unsigned ne_cur = __ballot_sync(0xffffffffu, lane < nsp && sb < se);
@@ -345,6 +352,7 @@ k_fused_push_moments(const __grid_constant__ FusedArgs a)
             const bool stray = phase1(g, sp, cur, lane < nb, p0 + lane, sp.beta, dt, dci, dcj, dck, fld, stcol, my_leavers);
             // global loads of the next batch fly during phase 2
             if (in_state == 1 || in_state == 2) load_batch(a.sp[in_s], in_p0, in_nb, lane, in);
+            if (in_state != 1 && has_next) { load_fields(ni, nj, nk, f0, f1); fld_ready = true; }
             const unsigned smask = __ballot_sync(0xffffffffu, stray);
             if (smask) {
                 uint32_t base = 0;
@@ -355,6 +363,7 @@ k_fused_push_moments(const __grid_constant__ FusedArgs a)
             __syncwarp();
 
             // ---- phase 2: contractions over the batch, four particles per step (columns >= nb hold c = 0, Wq = 0) ----
+#ifndef ECPUSH_DBG_NO_PHASE2
             {
                 const int ng = nb > 28 ? 8 : (nb + 3) >> 2;
 #pragma unroll 1
@@ -375,6 +384,7 @@ k_fused_push_moments(const __grid_constant__ FusedArgs a)
                     }
                 }
             }
+#endif
             __syncwarp();
 
             // ---- end of a species in this cell: its rho/Jhat corner sums, straight from the fragment ----
