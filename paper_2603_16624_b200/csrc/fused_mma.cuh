@@ -127,6 +127,16 @@ __device__ __forceinline__ uint32_t range_bound(const FusedArgs& a, uint32_t w, 
 
 struct ParticleRegs { double x, y, z, u, v, w, q; };
 
+__device__ __forceinline__ void load_batch(const SpeciesDev& sp, uint32_t p0, int nb, int lane, ParticleRegs& r)
+{
+    if (lane < nb) {
+        const uint32_t p = p0 + lane;
+        r.x = sp.x[p]; r.y = sp.y[p]; r.z = sp.z[p];
+        r.u = sp.u[p]; r.v = sp.v[p]; r.w = sp.w[p];
+        r.q = __ldg(sp.q + p);
+    }
+}
+
 // Phase 1 for one lane: returns true if the lane holds a stray.  `st` = staging tile + lane (the
 // lane's column), `fld` = the cell's corner fields, (dci,dcj,dck) = the cell's integer coordinates.
 __device__ __forceinline__ bool phase1(const Geom& g, const SpeciesDev& sp, const ParticleRegs& r, bool active,
