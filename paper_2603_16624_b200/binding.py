@@ -58,6 +58,7 @@ _PROTOS = {
     "ecsim_set_variant": (_c.c_int, [_P, _c.c_int]),
     "ecsim_set_resort_fraction": (_c.c_int, [_P, _c.c_double]),
     "ecsim_set_fused_warps": (_c.c_int, [_P, _c.c_int]),
+    "ecsim_set_slabs": (_c.c_int, [_P, _c.c_int]),
     "ecsim_enable_timing": (_c.c_int, [_P, _c.c_int]),
     "ecsim_kernel_ms": (_c.c_int, [_P, _c.POINTER(_c.c_float)]),
     "ecsim_launch_count": (_c.c_int64, [_P]),
@@ -202,6 +203,9 @@ class Ecsim:
 
     def set_fused_warps(self, w: int):
         _check(self.L.ecsim_set_fused_warps(self.h, w), "ecsim_set_fused_warps")
+
+    def set_slabs(self, n: int):
+        _check(self.L.ecsim_set_slabs(self.h, n), "ecsim_set_slabs")
 
     def enable_timing(self, on: bool = True):
         _check(self.L.ecsim_enable_timing(self.h, 1 if on else 0), "ecsim_enable_timing")

@@ -32,6 +32,8 @@ static int cuda_fail(cudaError_t e, const char* what, int line)
     } while (0)
 #define CK_LAUNCH() CK(cudaGetLastError())
 
+#define ECSIM_MAX_SLABS 16
+
 enum SortState { ST_UNSORTED = 0, ST_DECLARED = 1, ST_SEGMENTED = 2 };
 
 struct SpeciesHost {
@@ -69,6 +71,10 @@ struct ecsim_ctx {
     Geom g;
     int n_species = 0;
     cudaStream_t stream = nullptr;
+    cudaStream_t aux = nullptr;               // expansion of slab s-1 runs here while slab s is in the fused kernel
+    cudaEvent_t ev_slab[ECSIM_MAX_SLABS] = {};
+    cudaEvent_t ev_aux_done = nullptr;
+    int slabs = 0;                            // 0 = automatic
     SpeciesHost* sp = nullptr;
     Workspace ws;
     int variant = ECSIM_VARIANT_FUSED;
@@ -179,6 +185,10 @@ extern "C" int ecsim_init_grid(ecsim_ctx** ctx, int nx, int ny, int nz, double d
     c->sm_count = prop.multiProcessorCount;
     cudaError_t e = cudaEventCreate(&c->ev0);
     if (e == cudaSuccess) e = cudaEventCreate(&c->ev1);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->aux, cudaStreamNonBlocking);
+    for (int k = 0; k < ECSIM_MAX_SLABS && e == cudaSuccess; ++k)
+        e = cudaEventCreateWithFlags(&c->ev_slab[k], cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_aux_done, cudaEventDisableTiming);
     for (int s = 0; s < n_species && e == cudaSuccess; ++s)
         e = cudaEventCreateWithFlags(&c->sp[s].leavers_event, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaMallocHost(&c->h_leavers, sizeof(unsigned long long) * n_species);
@@ -203,6 +213,10 @@ extern "C" int ecsim_destroy(ecsim_ctx* c)
     }
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
+    for (int k = 0; k < ECSIM_MAX_SLABS; ++k)
+        if (c->ev_slab[k]) cudaEventDestroy(c->ev_slab[k]);
+    if (c->ev_aux_done) cudaEventDestroy(c->ev_aux_done);
+    if (c->aux) cudaStreamDestroy(c->aux);
     if (c->h_leavers) cudaFreeHost(c->h_leavers);
     if (c->h_strays) cudaFreeHost(c->h_strays);
     delete c;
@@ -385,6 +399,13 @@ extern "C" int ecsim_set_fused_warps(ecsim_ctx* c, int warps)
     return ECSIM_OK;
 }
 
+extern "C" int ecsim_set_slabs(ecsim_ctx* c, int slabs)
+{
+    if (!c || slabs < 0 || slabs > ECSIM_MAX_SLABS) return ECSIM_ERR_INVALID_ARG;
+    c->slabs = slabs;
+    return ECSIM_OK;
+}
+
 extern "C" int ecsim_enable_timing(ecsim_ctx* c, int on)
 {
     if (!c) return ECSIM_ERR_INVALID_ARG;
@@ -424,7 +445,7 @@ static cudaError_t launch_fused(const ecsim_ctx* c, const FusedArgs& fa)
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    const size_t cells = (size_t)c->g.nodes;
+    const size_t cells = (size_t)(fa.c_end - fa.c_begin);
     size_t grid = (cells + NW - 1) / NW;
     if (grid > (size_t)c->sm_count) grid = (size_t)c->sm_count;
     k_fused_push_moments<NW><<<(int)grid, NW * 32, smem, c->stream>>>(fa);
@@ -509,8 +530,6 @@ static int push_and_moments_impl(ecsim_ctx* c, int n_list, const int* list, cons
 
     FusedArgs fa;
     fa.g = g; fa.n_species = n_list; fa.E = E; fa.B = B; fa.dt = dt; fa.AM = w.AM;
-    fa.weight_total = (unsigned long long)CELL_WEIGHT * cells;
-    for (int i = 0; i < n_list; ++i) fa.weight_total += (unsigned long long)c->sp[list[i]].n;
     for (int i = 0; i < n_list; ++i) {
         const int s = list[i];
         SpeciesHost& sp = c->sp[s];
@@ -524,29 +543,65 @@ static int push_and_moments_impl(ecsim_ctx* c, int n_list, const int* list, cons
         d.stray_count = w.stray_count + s;
         d.leavers = w.leavers + s;
     }
-    if (c->timing) CK(cudaEventRecord(c->ev0, c->stream));
-    cudaError_t e;
-    if (c->fused_warps == 8) e = launch_fused<8>(c, fa);
-    else if (c->fused_warps == 12) e = launch_fused<12>(c, fa);
-    else e = launch_fused<16>(c, fa);
-    if (e != cudaSuccess) return cuda_fail(e, "k_fused_push_moments launch", __LINE__);
-    c->launches++;
-    if (c->timing) { CK(cudaEventRecord(c->ev1, c->stream)); c->ev_valid = true; }
 
-    // per-cell classes -> node arrays
-    if (M) {
-        ExpandArgs ea{g, w.AM, M, acc_M};
-        const long long blocks = (long long)g.nx * g.ny * ((g.nz + EXPAND_Z - 1) / EXPAND_Z);
-        k_expand_M<<<(unsigned)blocks, 256, 0, c->stream>>>(ea);
-        CK_LAUNCH();
+    // Slabs of x-planes: the fused kernel of slab s (main stream) overlaps the expansion of slab s-1
+    // (aux stream): the first is bound by FP64 issue, the second by HBM.  Node plane i needs the cell
+    // planes i-1 and i, so slab s expands its own planes; plane 0 (which needs plane nx-1) goes last.
+    int n_slabs = c->slabs;
+    if (n_slabs == 0) n_slabs = g.nodes >= (1 << 20) ? 8 : 1;
+    if (n_slabs > g.nx) n_slabs = g.nx;
+    const size_t plane = (size_t)g.ny * g.nz;
+    const int zchunks = (g.nz + EXPAND_Z - 1) / EXPAND_Z;
+    auto expand_planes = [&](int i0, int i1, cudaStream_t st) -> int {
+        if (i1 <= i0) return ECSIM_OK;
+        if (M) {
+            ExpandArgs ea{g, w.AM, M, acc_M, i0};
+            k_expand_M<<<(unsigned)((size_t)(i1 - i0) * g.ny * zchunks), 256, 0, st>>>(ea);
+            CK_LAUNCH();
+            c->launches++;
+        }
+        for (int i = 0; i < n_list && (rho || J); ++i) {
+            ExpandJArgs ja{g, fa.sp[i].AJ, rho ? rho + i * rho_stride : nullptr, J ? J + i * J_stride : nullptr, acc_J,
+                           (long long)(i0 * plane), (long long)(i1 * plane)};
+            k_expand_rhoJ<<<(unsigned)(((size_t)(i1 - i0) * plane + 255) / 256), 256, 0, st>>>(ja);
+            CK_LAUNCH();
+            c->launches++;
+        }
+        return ECSIM_OK;
+    };
+    // With slabs the fused kernels stay on the caller's stream, 12 warps x 128 registers per SM, and the
+    // expansions go to the context's second stream: one 256-thread expansion CTA fits beside a fused CTA on
+    // every SM.  (Measured alternatives, both slower: fused kernels on a high-priority stream with 8-24 SMs
+    // left free for the expansion; 16-warp fused CTAs, which leave no registers for an expansion CTA.)
+    const bool overlap = n_slabs > 1;
+    const int warps = overlap ? 12 : c->fused_warps;
+    if (c->timing) CK(cudaEventRecord(c->ev0, c->stream));
+    for (int sl = 0; sl < n_slabs; ++sl) {
+        const int i0 = (int)((long long)g.nx * sl / n_slabs), i1 = (int)((long long)g.nx * (sl + 1) / n_slabs);
+        fa.c_begin = (uint32_t)(i0 * plane);
+        fa.c_end = (uint32_t)(i1 * plane);
+        cudaError_t e;
+        if (warps == 8) e = launch_fused<8>(c, fa);
+        else if (warps == 12) e = launch_fused<12>(c, fa);
+        else e = launch_fused<16>(c, fa);
+        if (e != cudaSuccess) return cuda_fail(e, "k_fused_push_moments launch", __LINE__);
         c->launches++;
+        if (overlap) {
+            CK(cudaEventRecord(c->ev_slab[sl], c->stream));
+            CK(cudaStreamWaitEvent(c->aux, c->ev_slab[sl], 0));
+            rc = expand_planes(sl == 0 ? 1 : i0, i1, c->aux);
+            if (rc) return rc;
+        }
     }
-    for (int i = 0; i < n_list; ++i) {
-        if (!rho && !J) break;
-        ExpandJArgs ja{g, fa.sp[i].AJ, rho ? rho + i * rho_stride : nullptr, J ? J + i * J_stride : nullptr, acc_J};
-        k_expand_rhoJ<<<(unsigned)((g.nodes + 255) / 256), 256, 0, c->stream>>>(ja);
-        CK_LAUNCH();
-        c->launches++;
+    if (c->timing) { CK(cudaEventRecord(c->ev1, c->stream)); c->ev_valid = true; }
+    if (overlap) {
+        rc = expand_planes(0, 1, c->aux);
+        if (rc) return rc;
+        CK(cudaEventRecord(c->ev_aux_done, c->aux));
+        CK(cudaStreamWaitEvent(c->stream, c->ev_aux_done, 0));
+    } else {
+        rc = expand_planes(0, g.nx, c->stream);
+        if (rc) return rc;
     }
     // strays: the atomic path adds them to the node arrays (after the expansion wrote them)
     for (int i = 0; i < n_list; ++i) {

@@ -24,6 +24,7 @@ struct ExpandArgs {
     const double* AM;   // [cells][AM_PER_CELL]
     double* M;          // [nodes][27][3][3]
     int accumulate;
+    int i0;             // first node plane (x index) of this launch; the grid covers planes i0, i0+1, ...
 };
 
 // neighbour slots ordered by (x-y terms, z terms) = (4,2) | (4,1) | (2,2) | (2,1) | (1,2) | (1,1)
@@ -75,7 +76,7 @@ k_expand_M(const __grid_constant__ ExpandArgs a)
     const int zchunks = (g.nz + EXPAND_Z - 1) / EXPAND_Z;
     const int zc = (int)(blockIdx.x % (unsigned)zchunks);
     const int j = (int)((blockIdx.x / (unsigned)zchunks) % (unsigned)g.ny);
-    const int i = (int)(blockIdx.x / ((unsigned)zchunks * (unsigned)g.ny));
+    const int i = a.i0 + (int)(blockIdx.x / ((unsigned)zchunks * (unsigned)g.ny));
     const int im1 = i ? i - 1 : g.nx - 1, jm1 = j ? j - 1 : g.ny - 1;
     const int ebase = ij < 8 ? ij : AM_A8, emul = ij < 8 ? 8 : 1;
 
@@ -118,14 +119,15 @@ struct ExpandJArgs {
     double* rho;        // [nodes] or null
     double* J;          // [3][nodes] or null
     int accumulate;
+    long long n0, n1;   // nodes [n0, n1) of this launch
 };
 
 __global__ void __launch_bounds__(256)
 k_expand_rhoJ(ExpandJArgs a)
 {
     const Geom& g = a.g;
-    const long long node = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (node >= g.nodes) return;
+    const long long node = a.n0 + (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (node >= a.n1) return;
     const int k = (int)(node % g.nz);
     const int j = (int)((node / g.nz) % g.ny);
     const int i = (int)(node / ((long long)g.nz * g.ny));

@@ -71,7 +71,7 @@ struct FusedArgs {
     const double *E, *B;
     double dt;
     double* AM;                      // [cells][AM_PER_CELL]
-    unsigned long long weight_total; // sum of particles of the listed species + CELL_WEIGHT * cells
+    uint32_t c_begin, c_end;         // cells [c_begin, c_end) of this launch (one slab of x-planes)
     SpeciesDev sp[ECSIM_MAX_SPECIES];
 };
 
@@ -108,19 +108,25 @@ __device__ __forceinline__ double rcp_ge1(double d)
     return fma(r, e, r);
 }
 
-// First cell of warp w's range: smallest c with  CELL_WEIGHT*c + sum_s start_s[c] >= w/W of the total.
-__device__ __forceinline__ uint32_t range_bound(const FusedArgs& a, uint32_t w, uint32_t W)
+// Schedule weight of the cells [0, c): CELL_WEIGHT per cell + its particles of every listed species.
+__device__ __forceinline__ unsigned long long cells_weight(const FusedArgs& a, uint32_t c)
 {
-    const uint32_t cells = (uint32_t)a.g.nodes;
-    if (w == 0) return 0;
-    if (w >= W) return cells;
-    const unsigned long long target = a.weight_total / W * w + (a.weight_total % W) * w / W;
-    uint32_t lo = 0, hi = cells;
+    unsigned long long f = (unsigned long long)CELL_WEIGHT * c;
+    for (int s = 0; s < a.n_species; ++s) f += __ldg(a.sp[s].start + c);
+    return f;
+}
+
+// First cell of warp w's range: smallest c in [c_begin, c_end] whose weight from c_begin reaches w/W of the launch's.
+__device__ __forceinline__ uint32_t range_bound(const FusedArgs& a, uint32_t w, uint32_t W, unsigned long long w0,
+                                                unsigned long long total)
+{
+    if (w == 0) return a.c_begin;
+    if (w >= W) return a.c_end;
+    const unsigned long long target = w0 + total / W * w + (total % W) * w / W;
+    uint32_t lo = a.c_begin, hi = a.c_end;
     while (lo < hi) {
         const uint32_t mid = lo + (hi - lo) / 2;
-        unsigned long long f = (unsigned long long)CELL_WEIGHT * mid;
-        for (int s = 0; s < a.n_species; ++s) f += __ldg(a.sp[s].start + mid);
-        if (f >= target) hi = mid; else lo = mid + 1;
+        if (cells_weight(a, mid) >= target) hi = mid; else lo = mid + 1;
     }
     return lo;
 }
@@ -223,7 +229,7 @@ __device__ __forceinline__ bool phase1(const Geom& g, const SpeciesDev& sp, cons
 }
 
 template <int NW>
-__global__ void __launch_bounds__(NW * 32, 1)
+__global__ void __maxnreg__(128)   // 128 registers: 16 warps fill the file, 12 leave room for an expansion CTA
 k_fused_push_moments(const __grid_constant__ FusedArgs a)
 {
     extern __shared__ __align__(16) double smem[];
@@ -240,7 +246,8 @@ k_fused_push_moments(const __grid_constant__ FusedArgs a)
     const int nsp = a.n_species;
     const double dt = a.dt;
     const uint32_t W = gridDim.x * NW, wid = blockIdx.x * NW + warp;
-    const uint32_t c_lo = range_bound(a, wid, W), c_hi = range_bound(a, wid + 1, W);
+    const unsigned long long w0 = cells_weight(a, a.c_begin), wtot = cells_weight(a, a.c_end) - w0;
+    const uint32_t c_lo = range_bound(a, wid, W, w0, wtot), c_hi = range_bound(a, wid + 1, W, w0, wtot);
     if (c_lo >= c_hi) return;
 
     // lane roles of phase 2: row r of the A / B tiles, particle k of a group of four
