@@ -40,8 +40,8 @@
 constexpr int ST_PITCH = 36;     // doubles per staging row: 32 particles + 4 (pitch = 4 mod 16: LDS.64 conflict-free)
 constexpr int ROW_C = 0;         // rows 0..26: the 27 classes, class = kx*9 + ky*3 + kz
 constexpr int ROW_WQ = 27;       // rows 27..34: q/V * W[8], corner = a*4 + b*2 + c (also the junk rows 27..31 of A tile 3)
-constexpr int ROW_BA = 35;       // rows 35..42: beta*alpha[0..7]
-constexpr int ROW_A8 = 43;       // row 43: beta*alpha[8]
+constexpr int ROW_BA = 35;       // rows 35..42: alpha[0..7]
+constexpr int ROW_A8 = 43;       // row 43: alpha[8]
 constexpr int ROW_ONE = 44;      // row 44: 1 (constant);  rows 45..47: alpha v^n
 constexpr int ROW_VH = 45;
 constexpr int ROW_BJ = 40;       // B tile of the rho/Jhat contraction: rows 40..47, useful columns 4..7 = (1, vhat)
@@ -150,11 +150,11 @@ __device__ __forceinline__ bool phase1(const Geom& g, const SpeciesDev& sp, cons
                                        const double* __restrict__ fld, double* __restrict__ st, unsigned& leavers)
 {
     // weights relative to the warp's cell; outside [0,1) => not in this cell
-    double xi = r.x * g.rdx - dci, eta = r.y * g.rdy - dcj, zeta = r.z * g.rdz - dck;
+    const double xi = r.x * g.rdx - dci, eta = r.y * g.rdy - dcj, zeta = r.z * g.rdz - dck;
     const bool inside = active && in_unit_interval(xi) && in_unit_interval(eta) && in_unit_interval(zeta);
-    // lanes without a particle of this cell compute on harmless numbers with zero charge
-    if (!inside) { xi = 0.5; eta = 0.5; zeta = 0.5; }
-    const double vx = inside ? r.u : 0.0, vy = inside ? r.v : 0.0, vz = inside ? r.w : 0.0;
+    // Lanes without a particle of this cell (ragged tail, strays) run the same code on whatever finite
+    // particle their registers hold, with zero charge: their class weights and corner weights are exact zeros.
+    const double vx = r.u, vy = r.v, vz = r.w;
     const double q = inside ? r.q : 0.0;
     const double wx0 = 1.0 - xi, wy0 = 1.0 - eta, wz0 = 1.0 - zeta;
     double Ex = 0, Ey = 0, Ez = 0, Bx = 0, By = 0, Bz = 0;
@@ -182,9 +182,9 @@ __device__ __forceinline__ bool phase1(const Geom& g, const SpeciesDev& sp, cons
     // deposit factors (pre-push x and v, L49): operands of the contractions, one column per particle
     {
         double* sb = st + ROW_BA * ST_PITCH;
-        sb[0 * ST_PITCH] = beta * a00; sb[1 * ST_PITCH] = beta * a01; sb[2 * ST_PITCH] = beta * a02;
-        sb[3 * ST_PITCH] = beta * a10; sb[4 * ST_PITCH] = beta * a11; sb[5 * ST_PITCH] = beta * a12;
-        sb[6 * ST_PITCH] = beta * a20; sb[7 * ST_PITCH] = beta * a21; sb[8 * ST_PITCH] = beta * a22;
+        sb[0 * ST_PITCH] = a00; sb[1 * ST_PITCH] = a01; sb[2 * ST_PITCH] = a02;
+        sb[3 * ST_PITCH] = a10; sb[4 * ST_PITCH] = a11; sb[5 * ST_PITCH] = a12;
+        sb[6 * ST_PITCH] = a20; sb[7 * ST_PITCH] = a21; sb[8 * ST_PITCH] = a22;
         double* sv = st + ROW_VH * ST_PITCH;
         sv[0 * ST_PITCH] = a00 * vx + a01 * vy + a02 * vz;
         sv[1 * ST_PITCH] = a10 * vx + a11 * vy + a12 * vz;
@@ -195,8 +195,9 @@ __device__ __forceinline__ bool phase1(const Geom& g, const SpeciesDev& sp, cons
         double* sw = st + ROW_WQ * ST_PITCH;
 #pragma unroll
         for (int k = 0; k < 8; ++k) sw[k * ST_PITCH] = qV * W[k];
-        // 27 classes: q/V * px[kx] * py[ky] * pz[kz]
-        const double qx0 = qV * wx0, qx1 = qV * xi;
+        // 27 classes: q beta/V * px[kx] * py[ky] * pz[kz]  (beta rides on the class weights, alpha stays unscaled)
+        const double qbV = qV * beta;
+        const double qx0 = qbV * wx0, qx1 = qbV * xi;
         const double px[3] = {qx0 * wx0, qx0 * xi, qx1 * xi};
         const double py[3] = {wy0 * wy0, wy0 * eta, eta * eta};
         const double pz0 = wz0 * wz0, pz1 = wz0 * zeta, pz2 = zeta * zeta;
