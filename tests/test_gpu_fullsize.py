@@ -1,0 +1,127 @@
+"""-m gpu parity at BASELINE.json's full headline size (configs[2]: 128^3 cells, 268,435,456 particles), in the
+launch configuration bench.py times (ecsim_push_and_moments_all from the cell-sorted state, library defaults:
+slab-pipelined fused kernel + expansion).
+
+The oracle cannot run 268 M particles in seconds, so it computes SAMPLED outputs one by one: for a 3x3x3 block
+of cells, the 8 nodes whose eight surrounding cells all lie in the block are fully determined by the block's
+particles.  The test copies exactly those particles (as generated on the device, before the step) to the host,
+runs the oracle on them on the full-size grid, and compares rho / Jhat / M at the 8 nodes and x / v of the
+block's particles.  Blocks sit in the interior, across the periodic corner, and across slab boundaries.
+Properties that hold at any size are checked on the whole arrays: charge conservation and M's mirror symmetry.
+"""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2603_16624_b200 as pk
+import workloads as wl
+from gpu_util import MOM_TOL, POS_TOL, VEL_TOL, assert_particles_close
+from util import PKEYS, grid_of
+
+pytestmark = pytest.mark.gpu
+
+BLOCKS = [(40, 77, 3), (126, 126, 126), (14, 0, 60), (15, 127, 127), (63, 31, 0), (0, 0, 0), (111, 5, 90)]
+
+
+def _block_cells(cfg, origin):
+    i0, j0, k0 = origin
+    cells = []
+    for di in range(3):
+        for dj in range(3):
+            for dk in range(3):
+                cells.append((((i0 + di) % cfg.nx) * cfg.ny + (j0 + dj) % cfg.ny) * cfg.nz + (k0 + dk) % cfg.nz)
+    return cells
+
+
+def _inner_nodes(cfg, origin):
+    i0, j0, k0 = origin
+    return [(((i0 + a) % cfg.nx) * cfg.ny + (j0 + b) % cfg.ny) * cfg.nz + (k0 + c) % cfg.nz
+            for a in (1, 2) for b in (1, 2) for c in (1, 2)]
+
+
+@pytest.fixture(scope="module")
+def full_step():
+    free, _ = torch.cuda.mem_get_info()
+    if free < 60e9:
+        pytest.skip("needs ~60 GB of device memory")
+    cfg = wl.config(2)
+    dev = torch.device("cuda")
+    E, B = wl.gen_fields(cfg, device=dev)
+    nsp = len(cfg.species)
+    parts = []
+    for s in range(nsp):
+        p = wl.gen_species(cfg, s, device=dev)
+        parts.append({k: p[k].contiguous() for k in PKEYS})
+        del p
+    torch.cuda.empty_cache()
+    ppc = cfg.ppc
+    # host copies of the sampled blocks' particles BEFORE the step (uniform config: cell c owns [c*ppc, (c+1)*ppc))
+    before = {}
+    for origin in BLOCKS:
+        idx = torch.cat([torch.arange(c * ppc, (c + 1) * ppc, device=dev) for c in _block_cells(cfg, origin)])
+        before[origin] = (idx, [{k: parts[s][k][idx].cpu().numpy().copy() for k in PKEYS} for s in range(nsp)])
+    qsum = [float(parts[s]["q"].sum()) for s in range(nsp)]
+    ctx = pk.Ecsim(*grid_of(cfg), nsp)
+    ctx.set_workspace(max(int(p["x"].numel()) for p in parts))
+    for s, sp in enumerate(cfg.species):
+        ctx.load_particles(s, sp.qom, parts[s], sorted=True)
+    rho = torch.full((nsp, cfg.nodes), float("nan"), dtype=torch.float64, device=dev)
+    J = torch.full((nsp, 3, cfg.nodes), float("nan"), dtype=torch.float64, device=dev)
+    M = torch.full((cfg.nodes, 27, 3, 3), float("nan"), dtype=torch.float64, device=dev)
+    ctx.push_and_moments_all(E, B, cfg.dt, cfg.theta, rho, J, M, accumulate=pk.ACC_NONE)
+    torch.cuda.synchronize()
+    assert ctx.stray_count() == 0
+    yield dict(cfg=cfg, E=E, B=B, parts=parts, before=before, rho=rho, J=J, M=M, qsum=qsum)
+    ctx.close()
+
+
+@pytest.mark.parametrize("origin", BLOCKS)
+def test_sampled_nodes_and_particles_match_oracle(full_step, origin):
+    f = full_step
+    cfg = f["cfg"]
+    idx, parts_np = f["before"][origin]
+    nodes = _inner_nodes(cfg, origin)
+    En, Bn = f["E"].cpu().numpy(), f["B"].cpu().numpy()
+    total = oracle.Moments(cfg.nodes)          # calloc-backed: only the touched pages are committed
+    for s, sp in enumerate(cfg.species):
+        m = oracle.Moments(cfg.nodes)
+        oracle.step(grid_of(cfg), sp.qom, cfg.dt, parts_np[s], En, Bn, m)
+        got_rho = f["rho"][s, nodes].cpu().numpy()
+        got_J = f["J"][s][:, nodes].cpu().numpy()
+        assert np.all(np.abs(got_rho - m.rho[nodes]) <= MOM_TOL * m.rho_abs[nodes]), f"rho species {s}"
+        assert np.all(np.abs(got_J - m.J[:, nodes]) <= MOM_TOL * m.J_abs[:, nodes]), f"Jhat species {s}"
+        total.M[nodes] += m.M[nodes]
+        total.M_abs[nodes] += m.M_abs[nodes]
+        got = {k: f["parts"][s][k][idx].cpu().numpy() for k in PKEYS}
+        assert_particles_close(got, parts_np[s], cfg, f"block {origin} species {s}")
+    got_M = f["M"][nodes].cpu().numpy()
+    err = np.abs(got_M - total.M[nodes])
+    assert np.all(np.isfinite(got_M))
+    assert np.all(err <= MOM_TOL * total.M_abs[nodes]), f"M at block {origin}: worst {err.max():.3e}"
+
+
+def test_charge_is_conserved_on_the_whole_grid(full_step):
+    f = full_step
+    cfg = f["cfg"]
+    V = cfg.dx * cfg.dy * cfg.dz
+    for s in range(len(cfg.species)):
+        total = float(f["rho"][s].sum()) * V
+        assert abs(total - f["qsum"][s]) <= 1e-11 * abs(f["qsum"][s])     # sum_g rho_g V_g = sum_p q_p (north-star)
+        assert bool(torch.isfinite(f["J"][s]).all())
+
+
+@pytest.mark.parametrize("off", [(1, 0, 0), (0, -1, 1), (1, 1, -1)])
+def test_mass_matrix_mirror_symmetry_on_the_whole_grid(full_step, off):
+    """M_NN' = M_N'N per component (L73, R11): M[g][o] = M[g + off(o)][26 - o]."""
+    f = full_step
+    cfg = f["cfg"]
+    o = (off[0] + 1) * 9 + (off[1] + 1) * 3 + (off[2] + 1)
+    M5 = f["M"].view(cfg.nx, cfg.ny, cfg.nz, 27, 9)
+    a = M5[:, :, :, o, :]
+    b = torch.roll(M5[:, :, :, 26 - o, :], shifts=(-off[0], -off[1], -off[2]), dims=(0, 1, 2))
+    scale = float(a.abs().max())
+    assert scale > 0
+    assert float((a - b).abs().max()) <= 1e-12 * scale
