@@ -4,33 +4,35 @@
 // Design:
 //   * One FP64 pipe bounds this path.  DFMA and DMMA share it (measured:
 //     34.1 / 37.1 / 32-33 TFLOP/s alone / alone / mixed), but one `mma.sync.m8n8k4.f64` carries 256
-//     FMAs in one issue slot with two operand registers per lane, where 256 DFMA-FMAs need 8 issue
-//     slots and, as rank-1 updates, ~100 operand doubles from shared memory.  Version 2 (DFMA) ran
-//     at 91 % of the shared-memory wavefront peak and 42 % of the FP64 pipe (profiles/r01a).
+//     FMAs in one instruction with two operand registers per lane, where 256 DFMA-FMAs as rank-1
+//     updates need ~100 operand doubles from shared memory.  Version 2 (DFMA) ran at 91 % of the
+//     shared-memory wavefront peak and 42 % of the FP64 pipe (profiles/r01a).  An FP64 instruction
+//     holds its scheduler's issue port for its pipe time (DMMA 16 cycles, DFMA 2; profiles/r01b), so
+//     every other instruction of this kernel costs FP64 throughput too: the code below is written
+//     for few instructions per particle.
 //   * One warp owns a contiguous range of cells, chosen from the segment tables so that every warp
-//     of the grid gets the same number of particles (+ a per-cell weight): a particle-balanced
-//     schedule that also serves non-uniform loads (Harris sheet).
+//     of the launch gets the same number of particles (+ a per-cell weight): a particle-balanced
+//     schedule that also serves non-uniform loads (Harris sheet).  A launch covers the cells
+//     [c_begin, c_end): one slab of x-planes (the host overlaps the expansion of the previous slab).
 //   * Per cell, all particles of all species of the call stream through the warp in batches of 32.
 //   * Phase 1, lane = particle, branch-free: CIC weights (L49, L131), gather of E^{n+theta}, B^n
 //     from the cell's 8 corner nodes staged in shared memory (L88, L133), alpha_p as nine scalars
 //     (Eq. 2), push (Eq. 6-8), and the per-particle factors of the deposits,
 //     written TRANSPOSED ([value][particle]) to a per-warp staging tile in shared memory:
-//         c[27]     = q/V * px[kx] py[ky] pz[kz],   p?[0..2] = (w0^2, w0 w1, w1^2)
-//         b[13]     = beta*alpha[0..7] | 1, (alpha v^n)[0..2], beta*alpha[8]
+//         c[27]  = q beta/V * px[kx] py[ky] pz[kz],   p?[0..2] = (w0^2, w0 w1, w1^2)
+//         Wq[8]  = q/V * W[corner];   alpha[9];   1;   vhat[3] = alpha v^n
 //     Only 27 distinct products W_pN W_pN' exist per particle (three per axis), so the 8x8 = 64
-//     (node, neighbour) pairs of Eq. (3) collapse onto 27 "classes" per cell; and because
-//     sum_N' W_pN' = 1, W_pN itself is the sum of the 8 classes that pair corner N with any N':
-//     rho and Jhat (Eq. 1) come out of the same class sums.  Lanes without a particle (ragged
-//     tail, strays) run the same code with q = 0, so their columns hold zeros.
-//   * Phase 2, the pre-reduction of same-cell particles (north-star (b)) as a tall-skinny
-//     contraction over the particle index:  C[class][col] += sum_p c[class](p) * b[col](p),
-//     32 x 16 padded from 27 x 13, as 4 x 2 tiles of m8n8k4 DMMA per group of 4 particles.  Lane
-//     (r = lane/4, k = lane%4) reads c[8mt + r] and b[8nt + r] of particle 4g + k: 6 conflict-free
-//     LDS.64 per 8 DMMA.  The accumulators are 16 doubles per lane.
-//   * At the end of a species in a cell the rho/Jhat columns are folded to the 8 corners (through
-//     shared memory) and written to AJ[species][cell][8][4]; at the end of a cell the mass-matrix
-//     columns are written straight from the fragments, coalesced, to AM[cell][288].  No atomics;
-//     the result is deterministic for a given particle order.
+//     (node, neighbour) pairs of Eq. (3) collapse onto 27 "classes" per cell.  Lanes without a
+//     particle of the cell (ragged tail, strays) run the same code with q = 0: zero columns.
+//   * Phase 2, the pre-reduction of same-cell particles (north-star (b)) as tall-skinny
+//     contractions over the particle index, four particles per step:
+//         accM[mt] (4 DMMA)  += c[8 mt + r]  x  alpha[0..7]       32 padded classes x 8
+//         acc8[mt] (4 DFMA)  += c[8 mt + r]  *  alpha[8]          on the A fragment already in registers
+//         accJ     (1 DMMA)  += Wq[8 corners] x (.., 1, vhat)     rho and Jhat per corner (Eq. 1)
+//     Lane (r = lane/4, k = lane%4) reads row X + r, particle 4g + k: conflict-free LDS.64.
+//   * End of a species in a cell: accJ goes straight from the fragment to AJ[species][cell][8][4].
+//     End of a cell: accM / acc8 go straight from the fragments, 16-byte coalesced, to AM[cell][288].
+//     No atomics; the result is deterministic for a given particle order.
 //   * k_expand_* (expand.cuh) then build the node arrays.
 //   * A particle found outside the cell whose segment it is stored in (a "stray") is skipped here,
 //     listed, and handled by the atomic path afterwards.
