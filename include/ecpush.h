@@ -135,7 +135,8 @@ int ecsim_push_and_moments_host(ecsim_ctx *ctx, int64_t n, double q_over_m, int 
 int ecsim_set_variant(ecsim_ctx *ctx, int variant);
 
 /* Tuning knobs: fraction of a species that may sit outside its cell segment before the next step re-sorts
- * (default 0.01); warps per CTA of the fused kernel (8, 12 or 16; default 16; 12 whenever slabs overlap). */
+ * (default 0.01); warps per CTA of the fused kernel (8, 12 or 16, with 224, 168 or 128 registers per thread;
+ * default 12; always 12 x 128 when slabs overlap). */
 int ecsim_set_resort_fraction(ecsim_ctx *ctx, double fraction);
 int ecsim_set_fused_warps(ecsim_ctx *ctx, int warps);
 /* Number of x-plane slabs the FUSED step is cut into (1..16; 0 = automatic: 8 for grids of >= 2^20 nodes, else 1).

@@ -84,7 +84,7 @@ struct ecsim_ctx {
     bool ev_valid = false;
     int64_t launches = 0;
     int sm_count = 0;
-    int fused_warps = 16;
+    int fused_warps = 12;
     unsigned long long* h_leavers = nullptr;  // pinned [n_species]
     uint32_t* h_strays = nullptr;             // pinned [n_species]
     int last_call_species[ECSIM_MAX_SPECIES];
@@ -435,20 +435,20 @@ extern "C" int64_t ecsim_stray_count(ecsim_ctx* c)
     return total;
 }
 
-template <int NW>
+template <int NW, int REGS>
 static cudaError_t launch_fused(const ecsim_ctx* c, const FusedArgs& fa)
 {
     const size_t smem = (size_t)NW * WARP_SMEM_DOUBLES * sizeof(double);
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_fused_push_moments<NW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(k_fused_push_moments<NW, REGS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         configured = true;
     }
     const size_t cells = (size_t)(fa.c_end - fa.c_begin);
     size_t grid = (cells + NW - 1) / NW;
     if (grid > (size_t)c->sm_count) grid = (size_t)c->sm_count;
-    k_fused_push_moments<NW><<<(int)grid, NW * 32, smem, c->stream>>>(fa);
+    k_fused_push_moments<NW, REGS><<<(int)grid, NW * 32, smem, c->stream>>>(fa);
     return cudaGetLastError();
 }
 
@@ -574,16 +574,18 @@ static int push_and_moments_impl(ecsim_ctx* c, int n_list, const int* list, cons
     // every SM.  (Measured alternatives, both slower: fused kernels on a high-priority stream with 8-24 SMs
     // left free for the expansion; 16-warp fused CTAs, which leave no registers for an expansion CTA.)
     const bool overlap = n_slabs > 1;
-    const int warps = overlap ? 12 : c->fused_warps;
+    const int warps = c->fused_warps;
     if (c->timing) CK(cudaEventRecord(c->ev0, c->stream));
     for (int sl = 0; sl < n_slabs; ++sl) {
         const int i0 = (int)((long long)g.nx * sl / n_slabs), i1 = (int)((long long)g.nx * (sl + 1) / n_slabs);
         fa.c_begin = (uint32_t)(i0 * plane);
         fa.c_end = (uint32_t)(i1 * plane);
         cudaError_t e;
-        if (warps == 8) e = launch_fused<8>(c, fa);
-        else if (warps == 12) e = launch_fused<12>(c, fa);
-        else e = launch_fused<16>(c, fa);
+        // with slabs: 12 warps x 128 registers leave 16384 registers for one 256-thread expansion CTA
+        if (overlap) e = launch_fused<12, 128>(c, fa);
+        else if (warps == 8) e = launch_fused<8, 224>(c, fa);
+        else if (warps == 16) e = launch_fused<16, 128>(c, fa);
+        else e = launch_fused<12, 168>(c, fa);
         if (e != cudaSuccess) return cuda_fail(e, "k_fused_push_moments launch", __LINE__);
         c->launches++;
         if (overlap) {

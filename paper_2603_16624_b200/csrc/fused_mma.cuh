@@ -231,8 +231,10 @@ __device__ __forceinline__ bool phase1(const Geom& g, const SpeciesDev& sp, cons
     return active && !inside;
 }
 
-template <int NW>
-__global__ void __maxnreg__(128)   // 128 registers: 16 warps fill the file, 12 leave room for an expansion CTA
+// REGS: register cap.  Measured on config 2 (whole grid, ms): 12 warps x 168 regs 11.89, 12 x 144 12.23, 16 x 128
+// 12.15, 12 x 128 12.88, 8 x 200 13.63; warp counts that are not a multiple of the 4 schedulers lose (14 x 128 13.58).
+template <int NW, int REGS>
+__global__ void __maxnreg__(REGS)   // 128 registers: 16 warps fill the file, 12 leave room for an expansion CTA
 k_fused_push_moments(const __grid_constant__ FusedArgs a)
 {
     extern __shared__ __align__(16) double smem[];
