@@ -136,13 +136,14 @@ int ecsim_set_variant(ecsim_ctx *ctx, int variant);
 
 /* Tuning knobs: fraction of a species that may sit outside its cell segment before the next step re-sorts
  * (default 0.01); warps per CTA of the fused kernel (8, 12 or 16, with 224, 168 or 128 registers per thread;
- * default 12; always 12 x 128 when slabs overlap). */
+ * default 12; always 12 x 144 when slabs overlap). */
 int ecsim_set_resort_fraction(ecsim_ctx *ctx, double fraction);
 int ecsim_set_fused_warps(ecsim_ctx *ctx, int warps);
-/* Number of x-plane slabs the FUSED step is cut into (1..16; 0 = automatic: 8 for grids of >= 2^20 nodes, else 1).
- * With more than one slab the expansion of slab s-1 (HBM bound; on a second stream owned by the context) runs
- * beside the fused kernel of slab s (FP64-issue bound; 12 warps per SM so that an expansion CTA fits next to it);
- * the caller's stream waits for both before later work on it starts.  Results do not depend on the number. */
+/* Number of x-plane slabs the FUSED step is cut into (1..16; 0 = default = 1).  With more than one slab the
+ * expansion of slab s-1 (HBM bound; on a second stream owned by the context) runs beside the fused kernel of slab s
+ * (FP64-issue bound; 12 warps x 144 registers so that an expansion CTA fits next to it on every SM); the caller's
+ * stream waits for both before later work on it starts.  Results do not depend on the number.  On B200 one slab is
+ * fastest; the knob stays for other grid shapes. */
 int ecsim_set_slabs(ecsim_ctx *ctx, int slabs);
 
 /* Instrumentation.  ecsim_enable_timing(1) records CUDA events around the deposit/push kernel of every

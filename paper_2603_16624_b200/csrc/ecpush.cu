@@ -14,6 +14,7 @@
 #include "atomic_path.cuh"
 #include "fused_mma.cuh"
 #include "expand.cuh"
+#include "expand_tma.cuh"
 #include "probe.cuh"
 
 // --------------------------------------------------------------------------------------------
@@ -33,6 +34,7 @@ static int cuda_fail(cudaError_t e, const char* what, int line)
 #define CK_LAUNCH() CK(cudaGetLastError())
 
 #define ECSIM_MAX_SLABS 16
+#define ECPUSH_OVERLAP_REGS 144   // 12 warps x 144 leave 10240 registers: one 128-thread x 64-register k_expand_M_stream CTA
 
 enum SortState { ST_UNSORTED = 0, ST_DECLARED = 1, ST_SEGMENTED = 2 };
 
@@ -548,15 +550,16 @@ static int push_and_moments_impl(ecsim_ctx* c, int n_list, const int* list, cons
     // (aux stream): the first is bound by FP64 issue, the second by HBM.  Node plane i needs the cell
     // planes i-1 and i, so slab s expands its own planes; plane 0 (which needs plane nx-1) goes last.
     int n_slabs = c->slabs;
-    if (n_slabs == 0) n_slabs = g.nodes >= (1 << 20) ? 8 : 1;
+    if (n_slabs == 0) n_slabs = 1;   // measured on config 2: 1 slab 14.4 ms, 4 slabs 15.0, 8 slabs 15.3
     if (n_slabs > g.nx) n_slabs = g.nx;
     const size_t plane = (size_t)g.ny * g.nz;
-    const int zchunks = (g.nz + EXPAND_Z - 1) / EXPAND_Z;
+    const bool overlap = n_slabs > 1;
     auto expand_planes = [&](int i0, int i1, cudaStream_t st) -> int {
         if (i1 <= i0) return ECSIM_OK;
         if (M) {
-            ExpandArgs ea{g, w.AM, M, acc_M, i0};
-            k_expand_M<<<(unsigned)((size_t)(i1 - i0) * g.ny * zchunks), 256, 0, st>>>(ea);
+            // one short-lived CTA per (i,j) column (persistent CTAs kept the next slab's fused launch waiting)
+            ExpandStreamArgs ea{g, w.AM, M, acc_M, i0, i1};
+            k_expand_M_stream<<<(i1 - i0) * g.ny, XS_THREADS, XS_SMEM_BYTES, st>>>(ea);
             CK_LAUNCH();
             c->launches++;
         }
@@ -569,11 +572,12 @@ static int push_and_moments_impl(ecsim_ctx* c, int n_list, const int* list, cons
         }
         return ECSIM_OK;
     };
-    // With slabs the fused kernels stay on the caller's stream, 12 warps x 128 registers per SM, and the
-    // expansions go to the context's second stream: one 256-thread expansion CTA fits beside a fused CTA on
-    // every SM.  (Measured alternatives, both slower: fused kernels on a high-priority stream with 8-24 SMs
-    // left free for the expansion; 16-warp fused CTAs, which leave no registers for an expansion CTA.)
-    const bool overlap = n_slabs > 1;
+    // With slabs (ecsim_set_slabs > 1) the fused kernels stay on the caller's stream as 12 warps x 144 registers,
+    // and the expansions go to the context's second stream: one 128-thread expansion CTA fits beside a fused CTA
+    // on every SM.  Measured on config 2 this overlap does not pay (1 slab 14.4 ms, 4 slabs 15.0, 8 slabs 15.3:
+    // the fused kernel is bound by instruction issue, so the expansion's instructions are not free, and it
+    // loses its 168-register schedule); the default is one slab.  Other measured alternatives, all slower: fused
+    // kernels on a high-priority stream with 8-24 SMs left free; persistent expansion CTAs.
     const int warps = c->fused_warps;
     if (c->timing) CK(cudaEventRecord(c->ev0, c->stream));
     for (int sl = 0; sl < n_slabs; ++sl) {
@@ -581,8 +585,7 @@ static int push_and_moments_impl(ecsim_ctx* c, int n_list, const int* list, cons
         fa.c_begin = (uint32_t)(i0 * plane);
         fa.c_end = (uint32_t)(i1 * plane);
         cudaError_t e;
-        // with slabs: 12 warps x 128 registers leave 16384 registers for one 256-thread expansion CTA
-        if (overlap) e = launch_fused<12, 128>(c, fa);
+        if (overlap) e = launch_fused<12, ECPUSH_OVERLAP_REGS>(c, fa);
         else if (warps == 8) e = launch_fused<8, 224>(c, fa);
         else if (warps == 16) e = launch_fused<16, 128>(c, fa);
         else e = launch_fused<12, 168>(c, fa);

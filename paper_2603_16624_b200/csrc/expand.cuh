@@ -9,23 +9,12 @@
 // and the 3-D term list of M[N][o] is the product of the three per-axis lists: 1, 2, 4 or 8 cells
 // (Eq. 3 summed over the particles of every cell that holds both N and N').
 //
-// k_expand_M: one CTA walks EXPAND_Z consecutive nodes of one (i,j) column; thread t < 243 owns one
-// element (o, ij).  Threads are ordered by the SHAPE of their term list ((x-y terms) x (z terms)) so that
-// a warp's load count is uniform and short, and every load of a node is issued before the first use
-// (straight-line code per shape: the memory-level parallelism the first version lacked, profiles/r01a).
+// k_expand_M_stream (expand_tma.cuh) builds M; the outputs of a node are taken in the order of EXPAND_ORDER,
+// i.e. by the SHAPE of their term list ((x-y terms) x (z terms)), so that the threads of a warp loop equally long.
+// k_expand_rhoJ (below) builds rho and Jhat: 8 corner sums per node.
 #pragma once
 #include "common.cuh"
 #include "fused_mma.cuh"
-
-constexpr int EXPAND_Z = 32;
-
-struct ExpandArgs {
-    Geom g;
-    const double* AM;   // [cells][AM_PER_CELL]
-    double* M;          // [nodes][27][3][3]
-    int accumulate;
-    int i0;             // first node plane (x index) of this launch; the grid covers planes i0, i0+1, ...
-};
 
 // neighbour slots ordered by (x-y terms, z terms) = (4,2) | (4,1) | (2,2) | (2,1) | (1,2) | (1,1)
 __device__ __constant__ unsigned char EXPAND_ORDER[27] = {
@@ -38,82 +27,6 @@ __device__ __constant__ unsigned char EXPAND_ORDER[27] = {
 
 // Offset, in doubles inside a cell's AM block, of (class, ij): 8*class + ij for ij < 8, AM_A8 + class for
 // ij = 8 -- additive in the per-axis parts of class = 9 clx + 3 cly + clz.
-template <int NXY, int NTZ>
-__device__ __forceinline__ void expand_nodes(const ExpandArgs& a, const double* const (&col)[4], int ezA, int ezB,
-                                             bool zA_is_prev, int nxy, int ntz, int k0, int k1,
-                                             double* __restrict__ dst0)
-{
-    const int nz = a.g.nz;
-#pragma unroll 2
-    for (int k = k0; k < k1; ++k) {
-        // z terms: A = first entry of the z list, B = second (cell k-1, class 2) when dz = 0
-        const int km1 = k ? k - 1 : nz - 1;
-        const int zA = (zA_is_prev ? km1 : k) * AM_PER_CELL + ezA, zB = km1 * AM_PER_CELL + ezB;
-        double v[NXY][NTZ];
-#pragma unroll
-        for (int t = 0; t < NXY; ++t) {
-            v[t][0] = __ldg(col[t] + zA);
-            if (NTZ == 2) v[t][1] = __ldg(col[t] + zB);
-        }
-        double s = a.accumulate ? dst0[(size_t)k * 243] : 0.0;
-#pragma unroll
-        for (int t = 0; t < NXY; ++t) {
-            s += t < nxy ? v[t][0] : 0.0;
-            if (NTZ == 2) s += (t < nxy && ntz == 2) ? v[t][1] : 0.0;
-        }
-        dst0[(size_t)k * 243] = s;
-    }
-}
-
-// <= 64 registers (it needs ~60: capped at 40 it runs 2.5x slower): one CTA fits beside a 12-warp x 128-register
-// fused CTA on every SM
-__global__ void __launch_bounds__(256, 4)
-k_expand_M(const __grid_constant__ ExpandArgs a)
-{
-    const int t = threadIdx.x;
-    if (t >= 243) return;
-    const Geom& g = a.g;
-    const int o = EXPAND_ORDER[t / 9], ij = t % 9;
-    const int dx = o / 9 - 1, dy = (o / 3) % 3 - 1, dz = o % 3 - 1;
-    const int zchunks = (g.nz + EXPAND_Z - 1) / EXPAND_Z;
-    const int zc = (int)(blockIdx.x % (unsigned)zchunks);
-    const int j = (int)((blockIdx.x / (unsigned)zchunks) % (unsigned)g.ny);
-    const int i = a.i0 + (int)(blockIdx.x / ((unsigned)zchunks * (unsigned)g.ny));
-    const int im1 = i ? i - 1 : g.nx - 1, jm1 = j ? j - 1 : g.ny - 1;
-    const int ebase = ij < 8 ? ij : AM_A8, emul = ij < 8 ? 8 : 1;
-
-    // x and y term lists: (cell index, class); d = 0: (own, 0), (previous, 2); d = +1: (own, 1); d = -1: (previous, 1)
-    const int ntx = dx == 0 ? 2 : 1, nty = dy == 0 ? 2 : 1, ntz = dz == 0 ? 2 : 1;
-    const int nxy = ntx * nty;
-    const double* col[4];
-#pragma unroll
-    for (int e = 0; e < 4; ++e) {
-        const int ee = e < nxy ? e : 0;                 // e >= nxy repeats term 0 (its value is not added)
-        const int ty = ee % nty, tx = ee / nty;
-        const int ci = tx == 0 ? (dx >= 0 ? i : im1) : im1, cx = tx == 0 ? (dx == 0 ? 0 : 1) : 2;
-        const int cj = ty == 0 ? (dy >= 0 ? j : jm1) : jm1, cy = ty == 0 ? (dy == 0 ? 0 : 1) : 2;
-        col[e] = a.AM + ((size_t)ci * g.ny + cj) * g.nz * AM_PER_CELL + (ebase + emul * (9 * cx + 3 * cy));
-    }
-    // z list: dz = 0: (cell k, class 0), (cell k-1, class 2); dz = +1: (cell k, class 1); dz = -1: (cell k-1, class 1)
-    const int ezA = emul * (dz == 0 ? 0 : 1), ezB = emul * 2;
-    const bool zA_is_prev = dz < 0;
-
-    const int k0 = zc * EXPAND_Z;
-    const int k1 = min(k0 + EXPAND_Z, g.nz);
-    double* dst0 = a.M + ((size_t)i * g.ny + j) * g.nz * 243 + (size_t)(o * 9 + ij);
-    // longest lists in the warp: warps 0..7 see (4,2), (2,2), (2,1), (2,1), (2,2), (1,2), (1,1), (1,1)
-    const unsigned am = __activemask();
-    const int wxy = __reduce_max_sync(am, nxy), wz = __reduce_max_sync(am, ntz);
-    if (wz == 2) {
-        if (wxy == 4) expand_nodes<4, 2>(a, col, ezA, ezB, zA_is_prev, nxy, ntz, k0, k1, dst0);
-        else if (wxy == 2) expand_nodes<2, 2>(a, col, ezA, ezB, zA_is_prev, nxy, ntz, k0, k1, dst0);
-        else expand_nodes<1, 2>(a, col, ezA, ezB, zA_is_prev, nxy, ntz, k0, k1, dst0);
-    } else {
-        if (wxy == 4) expand_nodes<4, 1>(a, col, ezA, ezB, zA_is_prev, nxy, ntz, k0, k1, dst0);
-        else if (wxy == 2) expand_nodes<2, 1>(a, col, ezA, ezB, zA_is_prev, nxy, ntz, k0, k1, dst0);
-        else expand_nodes<1, 1>(a, col, ezA, ezB, zA_is_prev, nxy, ntz, k0, k1, dst0);
-    }
-}
 
 struct ExpandJArgs {
     Geom g;
