@@ -83,14 +83,6 @@ __device__ __forceinline__ bool in_unit_interval(double t)
     return (unsigned)__double2hiint(t) < 0x3FF00000u;
 }
 
-// Periodic wrap with an integer fast-path test: for x >= +0 the order of doubles is the order of
-// their bit patterns, so "0 <= x < L" is one unsigned 64-bit compare (negatives and NaN fail it).
-__device__ __forceinline__ double wrap_fast(double x, double L)
-{
-    if ((unsigned long long)__double_as_longlong(x) < (unsigned long long)__double_as_longlong(L)) return x;
-    return wrap_periodic(x, L);
-}
-
 // D(8x8) += A(8x4) * B(4x8) in FP64.  Lane l holds A[l/4][l%4], B[l%4][l/4], D[l/4][2(l%4) + {0,1}].
 __device__ __forceinline__ void dmma_m8n8k4(double2& d, double a, double b)
 {
@@ -219,9 +211,12 @@ __device__ __forceinline__ bool phase1(const Geom& g, const SpeciesDev& sp, cons
     const double vbz = a20 * tx + a21 * ty + a22 * tz;
     const double un = 2.0 * vbx - vx, vn = 2.0 * vby - vy, wn = 2.0 * vbz - vz;
     if (inside) {
-        const double xn = wrap_fast(fma(dt, un, r.x), g.Lx);
-        const double yn = wrap_fast(fma(dt, vn, r.y), g.Ly);
-        const double zn = wrap_fast(fma(dt, wn, r.z), g.Lz);
+        double xn = fma(dt, un, r.x), yn = fma(dt, vn, r.y), zn = fma(dt, wn, r.z);
+        // for x >= +0 the order of doubles is the order of their bit patterns: "0 <= x < L" is one unsigned compare
+        const bool in_box = (unsigned long long)__double_as_longlong(xn) < (unsigned long long)__double_as_longlong(g.Lx) &&
+                            (unsigned long long)__double_as_longlong(yn) < (unsigned long long)__double_as_longlong(g.Ly) &&
+                            (unsigned long long)__double_as_longlong(zn) < (unsigned long long)__double_as_longlong(g.Lz);
+        if (!in_box) { xn = wrap_periodic(xn, g.Lx); yn = wrap_periodic(yn, g.Ly); zn = wrap_periodic(zn, g.Lz); }
         sp.u[p] = un; sp.v[p] = vn; sp.w[p] = wn;
         sp.x[p] = xn; sp.y[p] = yn; sp.z[p] = zn;
         const bool stays = in_unit_interval(xn * g.rdx - dci) && in_unit_interval(yn * g.rdy - dcj) &&
@@ -385,28 +380,25 @@ k_fused_push_moments(const __grid_constant__ FusedArgs a)
             __syncwarp();
 
             // ---- phase 2: contractions over the batch, four particles per step (columns >= nb hold c = 0, Wq = 0) ----
-#ifndef ECPUSH_DBG_NO_PHASE2
             {
+                auto group = [&](int gq) {
+                    const double* f = frag + gq * 4;
+                    const double b0 = f[ROW_BA * ST_PITCH], a8 = f[(ROW_A8 - fr) * ST_PITCH];
+                    const double wq = f[ROW_WQ * ST_PITCH], bj = f[ROW_BJ * ST_PITCH];
+#pragma unroll
+                    for (int mt = 0; mt < 4; ++mt) {
+                        const double av = f[(ROW_C + 8 * mt) * ST_PITCH];
+                        dmma_m8n8k4(accM[mt], av, b0);
+                        acc8[mt] = fma(av, a8, acc8[mt]);
+                    }
+                    dmma_m8n8k4(accJ, wq, bj);
+                };
+                // two groups per iteration; ng odd: the extra group reads valid columns whose c and Wq are zero.
+                // (Fully unrolled for full batches it ran 2 % slower.)
                 const int ng = nb > 28 ? 8 : (nb + 3) >> 2;
 #pragma unroll 1
-                for (int gq = 0; gq < ng; gq += 2) {
-#pragma unroll
-                    for (int h = 0; h < 2; ++h) {
-                        // ng odd: the extra group reads valid columns whose c and Wq are zero
-                        const double* f = frag + (gq + h) * 4;
-                        const double b0 = f[ROW_BA * ST_PITCH], a8 = f[(ROW_A8 - fr) * ST_PITCH];
-                        const double wq = f[ROW_WQ * ST_PITCH], bj = f[ROW_BJ * ST_PITCH];
-#pragma unroll
-                        for (int mt = 0; mt < 4; ++mt) {
-                            const double av = f[(ROW_C + 8 * mt) * ST_PITCH];
-                            dmma_m8n8k4(accM[mt], av, b0);
-                            acc8[mt] = fma(av, a8, acc8[mt]);
-                        }
-                        dmma_m8n8k4(accJ, wq, bj);
-                    }
-                }
+                for (int gq = 0; gq < ng; gq += 2) { group(gq); group(gq + 1); }
             }
-#endif
             __syncwarp();
 
             // ---- end of a species in this cell: its rho/Jhat corner sums, straight from the fragment ----
