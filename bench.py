@@ -41,7 +41,7 @@ FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 NORTH_STAR_ROOFLINE_PPS = min(8.0e12 / BYTES_PER_PARTICLE_CFG2, FP64_PEAK_TFLOPS * 1e12 / FLOP_PER_PARTICLE)
 # dram__bytes_read.sum + dram__bytes_write.sum of k_fused_push_moments per launch, from the ncu
 # --set full capture summarised in profiles/ (None until a capture of this workload exists)
-FUSED_DRAM_TRAFFIC_BYTES = 33.67e9   # profiles/r01b: 15.59 GB read + 18.08 GB written per step of configs[2]
+FUSED_DRAM_TRAFFIC_BYTES = 33.50e9   # profiles/r01c: 15.50 GB read + 18.00 GB written per launch on configs[2]
 
 
 def parse_args():
