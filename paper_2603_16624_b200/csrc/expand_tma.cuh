@@ -3,10 +3,10 @@
 //
 // A CTA of 128 threads walks one (i,j) column of nodes along z.  Node (i,j,k) needs the class sums of the
 // 8 cells (i-1..i, j-1..j, k-1..k): four cell columns, two consecutive z levels.  The four cells of one z level
-// are four contiguous 2304-byte blocks of AM; thread 0 requests them with cp.async.bulk into a ring of XS_RING
-// stages in shared memory, each stage signalled by an mbarrier (expect_tx = 9216 bytes).  The loads in flight
+// are four contiguous 1952-byte blocks of AM; thread 0 requests them with cp.async.bulk into a ring of XS_RING
+// stages in shared memory, each stage signalled by an mbarrier (expect_tx = 7808 bytes).  The loads in flight
 // therefore cost no registers and no issue slots, and shared memory -- not the register file -- sets how many
-// CTAs an SM holds (ring of 3 = 27.6 KB: 8 CTAs).  Per node every thread reads <= 8 terms per output from
+// CTAs an SM holds (ring of 3 = 23.4 KB: 9 CTAs).  Per node every thread reads <= 8 terms per output from
 // shared memory (term lists: expand.cuh) and writes its outputs with plain stores; only thread 0 polls the
 // mbarrier, the others wait in the hardware barrier; a second __syncthreads orders "everybody has read the
 // previous level" before its slot is refilled.
@@ -27,7 +27,7 @@ constexpr int XS_THREADS = XS_THREADS_N;
 constexpr int XS_RING = XS_RING_N;
 constexpr int XS_OUT = (243 + XS_THREADS - 1) / XS_THREADS;   // outputs per thread
 constexpr int XS_STAGE_DOUBLES = 4 * AM_PER_CELL;                       // cells (i,j), (i,j-1), (i-1,j), (i-1,j-1)
-constexpr int XS_STAGE_BYTES = XS_STAGE_DOUBLES * 8;                    // 9216
+constexpr int XS_STAGE_BYTES = XS_STAGE_DOUBLES * 8;                    // 7808
 constexpr int XS_SMEM_BYTES = XS_RING * XS_STAGE_BYTES + XS_RING * 8;   // ring + mbarriers
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }

@@ -31,7 +31,7 @@
 //         accJ     (1 DMMA)  += Wq[8 corners] x (.., 1, vhat)     rho and Jhat per corner (Eq. 1)
 //     Lane (r = lane/4, k = lane%4) reads row X + r, particle 4g + k: conflict-free LDS.64.
 //   * End of a species in a cell: accJ goes straight from the fragment to AJ[species][cell][8][4].
-//     End of a cell: accM / acc8 go straight from the fragments, 16-byte coalesced, to AM[cell][288].
+//     End of a cell: accM / acc8 go straight from the fragments, 16-byte coalesced, to AM[cell][244].
 //     No atomics; the result is deterministic for a given particle order.
 //   * k_expand_* (expand.cuh) then build the node arrays.
 //   * A particle found outside the cell whose segment it is stored in (a "stray") is skipped here,
@@ -50,8 +50,8 @@ constexpr int ROW_BJ = 40;       // B tile of the rho/Jhat contraction: rows 40.
 constexpr int ST_ROWS = 48;
 constexpr int FLD_DOUBLES = 48;  // 8 corners x (Ex,Ey,Ez,Bx,By,Bz)
 constexpr int WARP_SMEM_DOUBLES = ST_ROWS * ST_PITCH + FLD_DOUBLES;
-constexpr int AM_PER_CELL = 288; // [4 m-tiles][8 classes][8 alpha entries] + [32 classes] alpha[8]
-constexpr int AM_A8 = 256;
+constexpr int AM_PER_CELL = 244; // [27 classes][8 alpha entries] + [27 classes] alpha[8] + 1 pad: 1952 B, a 16-byte multiple
+constexpr int AM_A8 = 216;
 constexpr int AJ_PER_CELL = 32;
 constexpr unsigned CELL_WEIGHT = 8;   // schedule weight of a cell, in particles
 
