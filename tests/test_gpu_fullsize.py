@@ -23,7 +23,11 @@ from util import PKEYS, grid_of
 
 pytestmark = pytest.mark.gpu
 
-BLOCKS = [(40, 77, 3), (126, 126, 126), (14, 0, 60), (15, 127, 127), (63, 31, 0), (0, 0, 0), (111, 5, 90)]
+# (config, block origin): config 2 = the headline (uniform, 128^3); config 3 = Harris sheet (96x96x48, 23..252 ppc):
+# blocks in the dense sheet (j ~ 48), in the thin background, and across the periodic corner
+BLOCKS = {2: [(40, 77, 3), (126, 126, 126), (14, 0, 60), (15, 127, 127), (63, 31, 0), (0, 0, 0), (111, 5, 90)],
+          3: [(10, 46, 20), (94, 94, 46), (50, 2, 0), (0, 47, 47), (77, 60, 11)]}
+CASES = [(c, o) for c in sorted(BLOCKS, reverse=True) for o in BLOCKS[c]]   # config 2 last: the whole-grid tests reuse it
 
 
 def _block_cells(cfg, origin):
@@ -42,12 +46,20 @@ def _inner_nodes(cfg, origin):
             for a in (1, 2) for b in (1, 2) for c in (1, 2)]
 
 
-@pytest.fixture(scope="module")
-def full_step():
+_CACHE = {}
+
+
+def _full_step(idx):
+    """One full-size step of config `idx`, cached for the module (one config resident at a time)."""
+    if idx in _CACHE:
+        return _CACHE[idx]
+    for k in list(_CACHE):
+        _CACHE.pop(k)["ctx"].close()
+    torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info()
     if free < 60e9:
         pytest.skip("needs ~60 GB of device memory")
-    cfg = wl.config(2)
+    cfg = wl.config(idx)
     dev = torch.device("cuda")
     E, B = wl.gen_fields(cfg, device=dev)
     nsp = len(cfg.species)
@@ -57,12 +69,12 @@ def full_step():
         parts.append({k: p[k].contiguous() for k in PKEYS})
         del p
     torch.cuda.empty_cache()
-    ppc = cfg.ppc
-    # host copies of the sampled blocks' particles BEFORE the step (uniform config: cell c owns [c*ppc, (c+1)*ppc))
+    # host copies of the sampled blocks' particles BEFORE the step (cell c owns [start[c], start[c+1]) of the sorted arrays)
+    _, start = wl.cell_layout(cfg)
     before = {}
-    for origin in BLOCKS:
-        idx = torch.cat([torch.arange(c * ppc, (c + 1) * ppc, device=dev) for c in _block_cells(cfg, origin)])
-        before[origin] = (idx, [{k: parts[s][k][idx].cpu().numpy().copy() for k in PKEYS} for s in range(nsp)])
+    for origin in BLOCKS[idx]:
+        sel = torch.cat([torch.arange(int(start[c]), int(start[c + 1]), device=dev) for c in _block_cells(cfg, origin)])
+        before[origin] = (sel, [{k: parts[s][k][sel].cpu().numpy().copy() for k in PKEYS} for s in range(nsp)])
     qsum = [float(parts[s]["q"].sum()) for s in range(nsp)]
     ctx = pk.Ecsim(*grid_of(cfg), nsp)
     ctx.set_workspace(max(int(p["x"].numel()) for p in parts))
@@ -74,13 +86,26 @@ def full_step():
     ctx.push_and_moments_all(E, B, cfg.dt, cfg.theta, rho, J, M, accumulate=pk.ACC_NONE)
     torch.cuda.synchronize()
     assert ctx.stray_count() == 0
-    yield dict(cfg=cfg, E=E, B=B, parts=parts, before=before, rho=rho, J=J, M=M, qsum=qsum)
-    ctx.close()
+    _CACHE[idx] = dict(cfg=cfg, E=E, B=B, parts=parts, before=before, rho=rho, J=J, M=M, qsum=qsum, ctx=ctx)
+    return _CACHE[idx]
 
 
-@pytest.mark.parametrize("origin", BLOCKS)
-def test_sampled_nodes_and_particles_match_oracle(full_step, origin):
-    f = full_step
+@pytest.fixture(scope="module")
+def full_step():
+    yield _full_step(2)
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _release_cache():
+    yield
+    for k in list(_CACHE):
+        _CACHE.pop(k)["ctx"].close()
+    torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("idx,origin", CASES)
+def test_sampled_nodes_and_particles_match_oracle(idx, origin):
+    f = _full_step(idx)
     cfg = f["cfg"]
     idx, parts_np = f["before"][origin]
     nodes = _inner_nodes(cfg, origin)
