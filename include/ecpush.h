@@ -64,7 +64,7 @@ enum ecsim_variant {
                                  scalar contribution; correct for any particle order                    */
     ECSIM_VARIANT_FUSED = 1   /* default: cell-sorted particles, one warp per cell, per-cell register accumulators
                                  (27 weight-product classes x 9 + Jhat + rho) written once per cell with plain
-                                 stores and expanded to the node arrays; strays take the atomic path */
+                                 stores and expanded to the node arrays; strays are added to the per-cell accumulators of their true cell */
 };
 
 /* Create a context for a periodic grid of nx*ny*nz cells (each >= 2) with spacing dx,dy,dz (> 0).
@@ -110,7 +110,8 @@ int ecsim_cell_index(ecsim_ctx *ctx, int species, int32_t *cell_out);
  * With variant FUSED an unsorted species is sorted first (same effect as ecsim_sort_particles).  After the
  * call the species keeps its segment table; the kernel counts the particles that left their cell, and the
  * next call re-sorts first when that count exceeds ecsim_set_resort_fraction() * n (default 1 %), otherwise
- * the leavers are handled as strays by the atomic path.  (The count is read through pinned memory: the next
+ * the leavers are handled as strays (pushed one thread per particle, deposited with atomics into the per-cell
+ * accumulators of their true cell before the expansion).  (The count is read through pinned memory: the next
  * call waits for this call's kernels to finish before it decides.) */
 int ecsim_push_and_moments(ecsim_ctx *ctx, int species, const double *E_theta, const double *B,
                            double dt, double theta, double *rho, double *Jhat, double *M, int accumulate);

@@ -131,3 +131,103 @@ k_push_moments_atomic(AtomicArgs a)
         if (lane_id() == 0 && my_leavers) atomicAdd(a.leavers, (unsigned long long)my_leavers);
     }
 }
+
+// ---------------------------------------------------------------------------------------------
+// Strays of the fused variant, deposited into the PER-CELL accumulators of their true cell instead of the
+// node arrays: AM[cell][class][ij] and AJ[cell][corner][4] (layouts of fused_mma.cuh), after the fused kernel
+// stored them and before the expansion reads them.  A stray then costs 243 + 32 atomics on one contiguous
+// 2.2 KB block instead of 576 + 32 atomics spread over 8 node blocks of 1.9 KB each (16 KB of HBM
+// read-modify-write per stray: measured 16 ns per stray, profiles/r01d).  Push as in k_push_moments_atomic.
+struct StrayArgs {
+    Geom g;
+    const uint32_t* list;       // indices of the strays
+    const uint32_t* list_count; // device count
+    double *x, *y, *z, *u, *v, *w;
+    const double* q;
+    const double *E, *B;        // [3][nodes]
+    double beta, dt;
+    double* AM;                 // [cells][AM_PER_CELL]
+    double* AJ;                 // [cells][8][4] of this species
+    unsigned long long* leavers;
+};
+
+__global__ void __launch_bounds__(128)
+k_push_strays_to_cells(StrayArgs a, int am_per_cell, int am_a8)
+{
+    const Geom& g = a.g;
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    const size_t count = (size_t)*a.list_count;
+    unsigned my_leavers = 0;
+    for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < count; t += stride) {
+        const size_t p = a.list[t];
+        const double x = a.x[p], y = a.y[p], z = a.z[p];
+        const double vx = a.u[p], vy = a.v[p], vz = a.w[p];
+        const double q = a.q[p];
+        const double sx = x * g.rdx, sy = y * g.rdy, sz = z * g.rdz;
+        const int i0 = lower_node(sx, g.nx), j0 = lower_node(sy, g.ny), k0 = lower_node(sz, g.nz);
+        const int i1 = (i0 + 1 == g.nx) ? 0 : i0 + 1;
+        const int j1 = (j0 + 1 == g.ny) ? 0 : j0 + 1;
+        const int k1 = (k0 + 1 == g.nz) ? 0 : k0 + 1;
+        const double xi = sx - i0, eta = sy - j0, zeta = sz - k0;
+        const double wx[2] = {1.0 - xi, xi}, wy[2] = {1.0 - eta, eta}, wz[2] = {1.0 - zeta, zeta};
+        double W[8], Ep[3] = {0, 0, 0}, Bp[3] = {0, 0, 0};
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+            const int ia = (c >> 2) & 1, ib = (c >> 1) & 1, ic = c & 1;
+            W[c] = (wx[ia] * wy[ib]) * wz[ic];
+            const long long node = ((long long)(ia ? i1 : i0) * g.ny + (ib ? j1 : j0)) * g.nz + (ic ? k1 : k0);
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                Ep[d] += W[c] * __ldg(a.E + d * g.nodes + node);
+                Bp[d] += W[c] * __ldg(a.B + d * g.nodes + node);
+            }
+        }
+        // rotation matrix, Eq. (2) as nine scalars (L53, L135); (I x B) v = B x v
+        const double bx = a.beta * Bp[0], by = a.beta * Bp[1], bz = a.beta * Bp[2];
+        const double invD = 1.0 / (1.0 + (bx * bx + by * by + bz * bz));
+        double al[9];
+        al[0] = invD * (1.0 + bx * bx); al[1] = invD * (bx * by + bz); al[2] = invD * (bx * bz - by);
+        al[3] = invD * (bx * by - bz); al[4] = invD * (1.0 + by * by); al[5] = invD * (by * bz + bx);
+        al[6] = invD * (bx * bz + by); al[7] = invD * (by * bz - bx); al[8] = invD * (1.0 + bz * bz);
+        const double vh[3] = {al[0] * vx + al[1] * vy + al[2] * vz, al[3] * vx + al[4] * vy + al[5] * vz,
+                              al[6] * vx + al[7] * vy + al[8] * vz};
+        const double qV = q * g.invV, qbV = qV * a.beta;
+        const size_t cell = ((size_t)i0 * g.ny + j0) * g.nz + k0;
+        // rho / Jhat per corner of the cell (L147, Eq. 1)
+        double* aj = a.AJ + cell * 32;
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+            const double wq = qV * W[c];
+            atomicAdd(aj + c * 4 + 0, wq);
+            atomicAdd(aj + c * 4 + 1, wq * vh[0]);
+            atomicAdd(aj + c * 4 + 2, wq * vh[1]);
+            atomicAdd(aj + c * 4 + 3, wq * vh[2]);
+        }
+        // the 27 weight-product classes of the cell (Eq. 3): class = kx*9 + ky*3 + kz, p?[0..2] = (w0^2, w0 w1, w1^2)
+        const double px[3] = {wx[0] * wx[0], wx[0] * wx[1], wx[1] * wx[1]};
+        const double py[3] = {wy[0] * wy[0], wy[0] * wy[1], wy[1] * wy[1]};
+        const double pz[3] = {wz[0] * wz[0], wz[0] * wz[1], wz[1] * wz[1]};
+        double* am = a.AM + cell * am_per_cell;
+#pragma unroll 1
+        for (int cls = 0; cls < 27; ++cls) {
+            const double cf = qbV * ((px[cls / 9] * py[(cls / 3) % 3]) * pz[cls % 3]);
+#pragma unroll
+            for (int e = 0; e < 8; ++e) atomicAdd(am + cls * 8 + e, cf * al[e]);
+            atomicAdd(am + am_a8 + cls, cf * al[8]);
+        }
+        // mover, Eq. (6)-(8) with periodic wrap
+        const double tx = vx + a.beta * Ep[0], ty = vy + a.beta * Ep[1], tz = vz + a.beta * Ep[2];
+        const double un = 2.0 * (al[0] * tx + al[1] * ty + al[2] * tz) - vx;
+        const double vn = 2.0 * (al[3] * tx + al[4] * ty + al[5] * tz) - vy;
+        const double wn = 2.0 * (al[6] * tx + al[7] * ty + al[8] * tz) - vz;
+        a.u[p] = un; a.v[p] = vn; a.w[p] = wn;
+        a.x[p] = wrap_periodic(x + a.dt * un, g.Lx);
+        a.y[p] = wrap_periodic(y + a.dt * vn, g.Ly);
+        a.z[p] = wrap_periodic(z + a.dt * wn, g.Lz);
+        my_leavers += 1;   // a stray stays outside the segment it is stored in
+    }
+    if (a.leavers) {
+        my_leavers = __reduce_add_sync(0xffffffffu, my_leavers);
+        if (lane_id() == 0 && my_leavers) atomicAdd(a.leavers, (unsigned long long)my_leavers);
+    }
+}

@@ -605,14 +605,28 @@ static int push_and_moments_impl(ecsim_ctx* c, int n_list, const int* list, cons
         CK(cudaEventRecord(c->ev_aux_done, c->aux));
         CK(cudaStreamWaitEvent(c->stream, c->ev_aux_done, 0));
     } else {
+        // strays first: they are deposited into the per-cell accumulators of their true cells (one 2.2 KB block
+        // per stray instead of eight node blocks), then one expansion serves everybody
+        for (int i = 0; i < n_list; ++i) {
+            const SpeciesHost& sp = c->sp[list[i]];
+            if (sp.n == 0) continue;
+            StrayArgs a;
+            a.g = g; a.list = fa.sp[i].stray_list; a.list_count = fa.sp[i].stray_count;
+            a.x = sp.x; a.y = sp.y; a.z = sp.z; a.u = sp.u; a.v = sp.v; a.w = sp.w; a.q = sp.q;
+            a.E = E; a.B = B; a.beta = fa.sp[i].beta; a.dt = dt;
+            a.AM = w.AM; a.AJ = fa.sp[i].AJ; a.leavers = fa.sp[i].leavers;
+            k_push_strays_to_cells<<<c->sm_count * 4, 128, 0, c->stream>>>(a, AM_PER_CELL, AM_A8);
+            CK_LAUNCH();
+            c->launches++;
+        }
         rc = expand_planes(0, g.nx, c->stream);
         if (rc) return rc;
     }
-    // strays: the atomic path adds them to the node arrays (after the expansion wrote them)
+    // with slabs the expansions have run already: the strays go to the node arrays through the atomic path
     for (int i = 0; i < n_list; ++i) {
         const int s = list[i];
         SpeciesHost& sp = c->sp[s];
-        if (sp.n > 0) {
+        if (sp.n > 0 && overlap) {
             AtomicArgs a;
             a.g = g; a.n = (uint32_t)sp.n; a.list = fa.sp[i].stray_list; a.list_count = fa.sp[i].stray_count;
             a.x = sp.x; a.y = sp.y; a.z = sp.z; a.u = sp.u; a.v = sp.v; a.w = sp.w; a.q = sp.q;
