@@ -9,7 +9,9 @@
 // CTAs an SM holds (ring of 3 = 23.4 KB: 9 CTAs).  Per node every thread reads <= 8 terms per output from
 // shared memory (term lists: expand.cuh) and writes its outputs with plain stores; only thread 0 polls the
 // mbarrier, the others wait in the hardware barrier; a second __syncthreads orders "everybody has read the
-// previous level" before its slot is refilled.
+// previous level" before its slot is refilled.  Slots, mbarrier phases and output pointers advance incrementally
+// and the term loops are shaped per warp (the first version spent 640 warp instructions per node, 90 % of them
+// address arithmetic and divergence bookkeeping).
 // Measured on config 2 (whole grid, profiles/r01c): 2.0 ms with 128 threads x ring 3; 2.2 ms (128 x 4),
 // 2.4 ms (256 x 3), 2.8 ms (64 x 3), 3.2 ms (128 x 5); the register-staged k_expand_M it replaces: 2.95 ms.
 #pragma once
@@ -66,31 +68,35 @@ struct ExpandStreamArgs {
     int i0, i1;         // node planes [i0, i1) of this launch
 };
 
-// Stage G of a CTA's sequence: column item G / (nz+1), level q = G % (nz+1); q = 0 holds the cells at z = nz-1
-// (the "k-1" of node 0), q >= 1 the cells at z = q-1.
-__device__ __forceinline__ void xs_issue_stage(const ExpandStreamArgs& a, uint32_t G, uint32_t n_stages, int first_item,
-                                               int item_stride, double* ring, uint64_t* bars)
+__device__ __forceinline__ double lds_f64(uint32_t addr)
 {
-    if (G >= n_stages) return;
-    const Geom& g = a.g;
-    const int per_col = g.nz + 1;
-    const int item = first_item + (int)(G / per_col) * item_stride;
-    const int q = (int)(G % per_col);
-    const int i = a.i0 + item / g.ny, j = item % g.ny;
-    const int im1 = i ? i - 1 : g.nx - 1, jm1 = j ? j - 1 : g.ny - 1;
-    const int z = q ? q - 1 : g.nz - 1;
-    const int slot = (int)(G % XS_RING);
-    double* dst = ring + (size_t)slot * XS_STAGE_DOUBLES;
-    uint64_t* bar = bars + slot;
-    mbar_expect_tx(bar, XS_STAGE_BYTES);
-    const int ci[4] = {i, i, im1, im1}, cj[4] = {j, jm1, j, jm1};
-#pragma unroll
-    for (int c = 0; c < 4; ++c) {
-        const double* src = a.AM + (((size_t)ci[c] * g.ny + cj[c]) * g.nz + z) * AM_PER_CELL;
-        bulk_g2s(dst + c * AM_PER_CELL, src, AM_PER_CELL * 8, bar);
-    }
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+    return v;
 }
 
+// Sum of one output's terms at one node.  NXY / TWO are the warp-wide longest lists (warp-uniform: no divergence);
+// a lane with a shorter list reads its term 0 again and adds nothing.  offA / offB: byte addresses (shared space) of
+// the output's z-list entries in the stages that hold them; o[t]: byte offsets of its x-y terms inside a stage.
+template <int NXY, bool TWO>
+__device__ __forceinline__ double xs_sum(double s, uint32_t offA, uint32_t offB, const uint32_t (&o)[4], int nxy, bool two)
+{
+    double vA[NXY], vB[NXY];
+#pragma unroll
+    for (int t = 0; t < NXY; ++t) {
+        vA[t] = lds_f64(offA + o[t]);
+        if (TWO) vB[t] = lds_f64(offB + o[t]);
+    }
+#pragma unroll
+    for (int t = 0; t < NXY; ++t) {
+        s += t < nxy ? vA[t] : 0.0;
+        if (TWO) s += (t < nxy && two) ? vB[t] : 0.0;
+    }
+    return s;
+}
+
+// One CTA per (i,j) column of nodes; stage q = 0 holds the cells at z = nz-1 (the "k-1" of node 0), stage q >= 1 the
+// cells at z = q-1; node k reads stages k ("previous level") and k+1 ("own level"); stage q lives in slot q % XS_RING.
 __global__ void __launch_bounds__(XS_THREADS, 1024 / XS_THREADS)   // <= 64 registers
 k_expand_M_stream(const __grid_constant__ ExpandStreamArgs a)
 {
@@ -99,12 +105,25 @@ k_expand_M_stream(const __grid_constant__ ExpandStreamArgs a)
     uint64_t* bars = reinterpret_cast<uint64_t*>(xs_smem + (size_t)XS_RING * XS_STAGE_BYTES);
     const Geom& g = a.g;
     const int tid = threadIdx.x;
-    const int n_items = (a.i1 - a.i0) * g.ny;
-    const int first_item = blockIdx.x, item_stride = gridDim.x;
-    if (first_item >= n_items) return;
-    const int my_items = (n_items - first_item + item_stride - 1) / item_stride;
-    const int per_col = g.nz + 1;
-    const uint32_t n_stages = (uint32_t)my_items * (uint32_t)per_col;   // < 2^32: a CTA's columns x (nz + 1)
+    const int i = a.i0 + (int)(blockIdx.x / (unsigned)g.ny), j = (int)(blockIdx.x % (unsigned)g.ny);
+    const int im1 = i ? i - 1 : g.nx - 1, jm1 = j ? j - 1 : g.ny - 1;
+    const int n_stages = g.nz + 1;
+    // the four cell columns of this node column: (i,j), (i,j-1), (i-1,j), (i-1,j-1)
+    const double* colsrc[4] = {a.AM + ((size_t)i * g.ny + j) * g.nz * AM_PER_CELL,
+                               a.AM + ((size_t)i * g.ny + jm1) * g.nz * AM_PER_CELL,
+                               a.AM + ((size_t)im1 * g.ny + j) * g.nz * AM_PER_CELL,
+                               a.AM + ((size_t)im1 * g.ny + jm1) * g.nz * AM_PER_CELL};
+    auto issue = [&](int q) {      // thread 0 only
+        if (q >= n_stages) return;
+        const int z = q ? q - 1 : g.nz - 1;
+        const int slot = q % XS_RING;
+        uint64_t* bar = bars + slot;
+        mbar_expect_tx(bar, XS_STAGE_BYTES);
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+            bulk_g2s(ring + (size_t)slot * XS_STAGE_DOUBLES + c * AM_PER_CELL, colsrc[c] + (size_t)z * AM_PER_CELL,
+                     AM_PER_CELL * 8, bar);
+    };
 
     if (tid == 0) {
         for (int s = 0; s < XS_RING; ++s) mbar_init(bars + s, 1);
@@ -112,82 +131,76 @@ k_expand_M_stream(const __grid_constant__ ExpandStreamArgs a)
     }
     __syncthreads();
     if (tid == 0)
-        for (int s = 0; s < XS_RING; ++s) xs_issue_stage(a, s, n_stages, first_item, item_stride, ring, bars);
+        for (int s = 0; s < XS_RING; ++s) issue(s);
 
-    // the four outputs of this thread: elements e = tid + 64 m of the 243, in the order of EXPAND_ORDER.
-    // Packed per output: offsets (in doubles, inside a stage) of its <= 4 x-y terms, and its z list.
-    unsigned offs01[XS_OUT], offs23[XS_OUT], zinfo[XS_OUT];
-    int mbase[XS_OUT];
+    // the outputs of this thread: elements e = tid + XS_THREADS m of the 243, in the order of EXPAND_ORDER
+    uint32_t off[XS_OUT][4];       // byte offsets of the <= 4 x-y terms inside a stage (term 0 repeated when fewer)
+    uint32_t ezA[XS_OUT], ezB[XS_OUT];
+    int nxy[XS_OUT], wxy[XS_OUT];
+    bool two[XS_OUT], wtwo[XS_OUT], a_prev[XS_OUT], valid[XS_OUT];
+    double* mptr[XS_OUT];
 #pragma unroll
     for (int m = 0; m < XS_OUT; ++m) {
         const int e = tid + XS_THREADS * m;
-        const int ee = e < 243 ? e : 0;
+        valid[m] = e < 243;
+        const int ee = valid[m] ? e : 0;
         const int o = EXPAND_ORDER[ee / 9], ij = ee % 9;
         const int dx = o / 9 - 1, dy = (o / 3) % 3 - 1, dz = o % 3 - 1;
         const int ebase = ij < 8 ? ij : AM_A8, emul = ij < 8 ? 8 : 1;
-        const int ntx = dx == 0 ? 2 : 1, nty = dy == 0 ? 2 : 1, ntz = dz == 0 ? 2 : 1;
-        const int nxy = ntx * nty;
-        unsigned off[4];
+        const int ntx = dx == 0 ? 2 : 1, nty = dy == 0 ? 2 : 1;
+        nxy[m] = ntx * nty;
+        two[m] = dz == 0;
 #pragma unroll
         for (int t = 0; t < 4; ++t) {
-            const int tt = t < nxy ? t : 0;
+            const int tt = t < nxy[m] ? t : 0;
             const int ty = tt % nty, tx = tt / nty;
             // column slot = xsel*2 + ysel, sel 0 = own (i or j), 1 = previous
             const int xsel = tx == 0 ? (dx >= 0 ? 0 : 1) : 1, cx = tx == 0 ? (dx == 0 ? 0 : 1) : 2;
             const int ysel = ty == 0 ? (dy >= 0 ? 0 : 1) : 1, cy = ty == 0 ? (dy == 0 ? 0 : 1) : 2;
-            off[t] = (unsigned)((xsel * 2 + ysel) * AM_PER_CELL + ebase + emul * (9 * cx + 3 * cy));
+            off[m][t] = 8u * (unsigned)((xsel * 2 + ysel) * AM_PER_CELL + ebase + emul * (9 * cx + 3 * cy));
         }
-        offs01[m] = off[0] | (off[1] << 16);
-        offs23[m] = off[2] | (off[3] << 16);
         // z list: dz = 0: (own level, class 0), (previous level, class 2); dz = +1: (own, 1); dz = -1: (previous, 1)
-        const unsigned ezA = (unsigned)(emul * (dz == 0 ? 0 : 1)), ezB = (unsigned)(emul * 2);
-        zinfo[m] = ezA | (ezB << 8) | ((unsigned)nxy << 16) | ((unsigned)(ntz == 2) << 24) | ((unsigned)(dz < 0) << 25) |
-                   ((unsigned)(e < 243) << 26);
-        mbase[m] = o * 9 + ij;
+        ezA[m] = 8u * (unsigned)(emul * (dz == 0 ? 0 : 1));
+        ezB[m] = 8u * (unsigned)(emul * 2);
+        a_prev[m] = dz < 0;
+        mptr[m] = a.M + ((size_t)i * g.ny + j) * g.nz * 243 + (size_t)(o * 9 + ij);
+        // the warp's longest lists (whole warps take part: 128 threads)
+        wxy[m] = __reduce_max_sync(0xffffffffu, valid[m] ? nxy[m] : 1);
+        wtwo[m] = __any_sync(0xffffffffu, valid[m] && two[m]);
     }
 
-    uint32_t G = 0;     // stage holding the "previous level" of the node being computed
+    const uint32_t ring_s = smem_u32(ring);
+    int slot_prev = 0, slot_own = 1;          // stage k in slot k % XS_RING
+    uint32_t phase_bits = 0;                  // bit s: parity of the next wait on slot s
+    if (tid == 0) { mbar_wait(bars + 0, 0); phase_bits ^= 1u; }
 #pragma unroll 1
-    for (int it = 0; it < my_items; ++it) {
-        const int item = first_item + it * item_stride;
-        const int i = a.i0 + item / g.ny, j = item % g.ny;
-        double* mcol = a.M + ((size_t)i * g.ny + j) * g.nz * 243;
-        // level q = 0 of this column.  Only thread 0 polls the mbarriers; the others sit in the hardware barrier
-        // and take no issue slots from the fused CTA next door.
-        if (tid == 0) mbar_wait(bars + (int)(G % XS_RING), (unsigned)((G / XS_RING) & 1));
-#pragma unroll 1
-        for (int k = 0; k < g.nz; ++k) {
-            const uint32_t Gown = G + 1;
-            if (tid == 0) mbar_wait(bars + (int)(Gown % XS_RING), (unsigned)((Gown / XS_RING) & 1));
-            __syncthreads();
-            const double* prev = ring + (size_t)(G % XS_RING) * XS_STAGE_DOUBLES;
-            const double* own = ring + (size_t)(Gown % XS_RING) * XS_STAGE_DOUBLES;
-            double* mnode = mcol + (size_t)k * 243;
+    for (int k = 0; k < g.nz; ++k) {
+        // only thread 0 polls the mbarrier; the others wait in the hardware barrier and take no issue slots
+        if (tid == 0) { mbar_wait(bars + slot_own, (phase_bits >> slot_own) & 1u); phase_bits ^= 1u << slot_own; }
+        __syncthreads();
+        const uint32_t prev_s = ring_s + (uint32_t)slot_prev * XS_STAGE_BYTES;
+        const uint32_t own_s = ring_s + (uint32_t)slot_own * XS_STAGE_BYTES;
 #pragma unroll
-            for (int m = 0; m < XS_OUT; ++m) {
-                const unsigned zi = zinfo[m];
-                if (!((zi >> 26) & 1u)) continue;
-                const int nxy = (int)((zi >> 16) & 0xffu);
-                const double* zA = (((zi >> 25) & 1u) ? prev : own) + (zi & 0xffu);
-                const double* zB = prev + ((zi >> 8) & 0xffu);
-                const bool two = (zi >> 24) & 1u;
-                double s = a.accumulate ? mnode[mbase[m]] : 0.0;
-                const unsigned o4[4] = {offs01[m] & 0xffffu, offs01[m] >> 16, offs23[m] & 0xffffu, offs23[m] >> 16};
-#pragma unroll
-                for (int t = 0; t < 4; ++t) {
-                    if (t < nxy) {
-                        s += zA[o4[t]];
-                        if (two) s += zB[o4[t]];
-                    }
+        for (int m = 0; m < XS_OUT; ++m) {
+            if (valid[m]) {
+                const uint32_t offA = (a_prev[m] ? prev_s : own_s) + ezA[m], offB = prev_s + ezB[m];
+                double s = a.accumulate ? *mptr[m] : 0.0;
+                if (wtwo[m]) {
+                    if (wxy[m] == 4) s = xs_sum<4, true>(s, offA, offB, off[m], nxy[m], two[m]);
+                    else if (wxy[m] == 2) s = xs_sum<2, true>(s, offA, offB, off[m], nxy[m], two[m]);
+                    else s = xs_sum<1, true>(s, offA, offB, off[m], nxy[m], two[m]);
+                } else {
+                    if (wxy[m] == 4) s = xs_sum<4, false>(s, offA, offB, off[m], nxy[m], two[m]);
+                    else if (wxy[m] == 2) s = xs_sum<2, false>(s, offA, offB, off[m], nxy[m], two[m]);
+                    else s = xs_sum<1, false>(s, offA, offB, off[m], nxy[m], two[m]);
                 }
-                mnode[mbase[m]] = s;
+                *mptr[m] = s;
             }
-            __syncthreads();                                   // stage G has been read by everybody: refill its slot
-            if (tid == 0) xs_issue_stage(a, G + XS_RING, n_stages, first_item, item_stride, ring, bars);
-            G = Gown;
+            mptr[m] += 243;
         }
-        // the last level of the column is nobody's "previous" (the barrier above covers its readers): refill it too
-        if (tid == 0) xs_issue_stage(a, G + XS_RING, n_stages, first_item, item_stride, ring, bars);
-        G += 1;
+        __syncthreads();                                   // the previous level has been read by everybody: refill its slot
+        if (tid == 0) issue(k + XS_RING);
+        slot_prev = slot_own;
+        slot_own = slot_own + 1 == XS_RING ? 0 : slot_own + 1;
     }
 }
