@@ -44,6 +44,7 @@ struct SpeciesHost {
     double qom = 0.0;
     double *x = nullptr, *y = nullptr, *z = nullptr, *u = nullptr, *v = nullptr, *w = nullptr, *q = nullptr;
     int state = ST_UNSORTED;
+    bool nearly_sorted = false;     // the arrays were cell-sorted before the last pushes (a re-sort, not a first sort)
     bool leavers_pending = false;   // an async copy of the leaver counter is in flight
     cudaEvent_t leavers_event = nullptr;
 };
@@ -60,6 +61,9 @@ struct Workspace {
     uint32_t* rank = nullptr;        // [n_max]
     uint32_t* perm = nullptr;        // [n_max]
     double* spare = nullptr;         // [n_max]
+    uint32_t* tile_hist = nullptr;   // [buckets][tiles] of the two-step move of a random-order sort
+    uint32_t* tile_scan = nullptr;   // its exclusive scan (+1)
+    uint32_t* tile_sums = nullptr;   // block sums of that scan
     uint32_t* stray_list = nullptr;  // [n_species][n_max]
     double* AM = nullptr;            // [cells][243]
     double* AJ = nullptr;            // [n_species][cells][32]
@@ -121,6 +125,12 @@ static size_t carve(const ecsim_ctx* c, int64_t n_max, void* base, Workspace* ou
     w.rank = k.take<uint32_t>(n);
     w.perm = k.take<uint32_t>(n);
     w.spare = k.take<double>(n);
+    {
+        const size_t m = (size_t)SORT_MAX_BUCKETS * (n / SORT_TILE + 1);
+        w.tile_hist = k.take<uint32_t>(m);
+        w.tile_scan = k.take<uint32_t>(m + 1);
+        w.tile_sums = k.take<uint32_t>(m / SCAN_BLOCK + 2);
+    }
     w.stray_list = k.take<uint32_t>(nsp * n);
     w.AM = k.take<double>(cells * AM_PER_CELL);
     w.AJ = k.take<double>(nsp * cells * AJ_PER_CELL);
@@ -283,6 +293,7 @@ extern "C" int ecsim_load_particles(ecsim_ctx* c, int s, int64_t n, double q_ove
     sp.qom = q_over_m;
     sp.x = x; sp.y = y; sp.z = z; sp.u = u; sp.v = v; sp.w = w; sp.q = q;
     sp.state = sorted ? ST_DECLARED : ST_UNSORTED;
+    sp.nearly_sorted = sorted != 0;
     sp.leavers_pending = false;
     return ECSIM_OK;
 }
@@ -344,18 +355,61 @@ extern "C" int ecsim_sort_particles(ecsim_ctx* c, int s, int32_t* cell_count_out
     if (sp.n > 0) {
         const uint32_t n = (uint32_t)sp.n;
         const int grid = grid_for(c, (size_t)sp.n, 256, 16);
-        k_build_perm<<<grid, 256, 0, c->stream>>>(n, w.cell, w.rank, start, w.perm);
-        CK_LAUNCH();
-        c->launches++;
         double* arrays[7] = {sp.x, sp.y, sp.z, sp.u, sp.v, sp.w, sp.q};
-        for (int a = 0; a < 7; ++a) {
-            k_gather_f64<<<grid, 256, 0, c->stream>>>(n, w.perm, arrays[a], w.spare);
+        if (sp.nearly_sorted) {
+            // a re-sort after pushes: perm is close to the identity, the gather reads almost sequentially
+            k_build_perm<<<grid, 256, 0, c->stream>>>(n, w.cell, w.rank, start, w.perm);
             CK_LAUNCH();
-            CK(cudaMemcpyAsync(arrays[a], w.spare, sizeof(double) * (size_t)n, cudaMemcpyDeviceToDevice, c->stream));
-            c->launches += 2;
+            c->launches++;
+            for (int a = 0; a < 7; ++a) {
+                k_gather_f64<<<grid, 256, 0, c->stream>>>(n, w.perm, arrays[a], w.spare);
+                CK_LAUNCH();
+                CK(cudaMemcpyAsync(arrays[a], w.spare, sizeof(double) * (size_t)n, cudaMemcpyDeviceToDevice, c->stream));
+                c->launches += 2;
+            }
+            if (perm_out)
+                CK(cudaMemcpyAsync(perm_out, w.perm, sizeof(uint32_t) * (size_t)n, cudaMemcpyDeviceToDevice, c->stream));
+        } else {
+            // arbitrary order: the bucketed two-step move of sort.cuh
+            static bool configured = false;
+            if (!configured) {
+                CK(cudaFuncSetAttribute(k_stage_to_slots, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SORT_STAGE_SMEM));
+                configured = true;
+            }
+            int shift = 13;
+            while ((((n - 1) >> shift) + 1) > (uint32_t)SORT_MAX_BUCKETS) ++shift;
+            const uint32_t nbk = ((n - 1) >> shift) + 1;
+            const uint32_t tiles = (n + SORT_TILE - 1) / SORT_TILE;
+            const uint32_t m = nbk * tiles;
+            uint32_t* dest = w.rank;                                   // rank -> dest in place
+            uint32_t* slot = reinterpret_cast<uint32_t*>(w.cell);      // the cell ids are not needed after that
+            uint32_t* perm2 = w.perm;
+            k_dest_and_tile_hist<<<tiles, 256, 0, c->stream>>>(n, w.cell, dest, start, shift, tiles, w.tile_hist);
+            CK_LAUNCH();
+            const uint32_t sb = (m + SCAN_BLOCK - 1) / SCAN_BLOCK;
+            k_scan_blocks<<<sb, SCAN_BLOCK, 0, c->stream>>>(w.tile_hist, w.tile_scan, w.tile_sums, m);
+            CK_LAUNCH();
+            k_scan_sums<<<1, SCAN_BLOCK, 0, c->stream>>>(w.tile_sums, sb, w.tile_scan, m);
+            CK_LAUNCH();
+            k_scan_add<<<sb, SCAN_BLOCK, 0, c->stream>>>(w.tile_scan, w.tile_sums, m);
+            CK_LAUNCH();
+            k_assign_slots<<<tiles, 256, 0, c->stream>>>(n, dest, w.tile_scan, shift, tiles, slot, perm2);
+            CK_LAUNCH();
+            c->launches += 5;
+            for (int a = 0; a < 7; ++a) {
+                k_stage_to_slots<<<tiles, SORT_STAGE_THREADS, SORT_STAGE_SMEM, c->stream>>>(
+                    n, dest, slot, w.tile_hist, w.tile_scan, shift, tiles, arrays[a], w.spare);
+                CK_LAUNCH();
+                k_gather_f64<<<grid, 256, 0, c->stream>>>(n, perm2, w.spare, arrays[a]);
+                CK_LAUNCH();
+                c->launches += 2;
+            }
+            if (perm_out) {
+                k_perm_from_dest<<<grid, 256, 0, c->stream>>>(n, dest, perm_out);
+                CK_LAUNCH();
+                c->launches++;
+            }
         }
-        if (perm_out)
-            CK(cudaMemcpyAsync(perm_out, w.perm, sizeof(uint32_t) * (size_t)n, cudaMemcpyDeviceToDevice, c->stream));
     }
     if (cell_count_out) {
         k_copy_u32_to_i32<<<grid_for(c, cells, 256, 8), 256, 0, c->stream>>>(cells, w.count, cell_count_out);
@@ -363,6 +417,7 @@ extern "C" int ecsim_sort_particles(ecsim_ctx* c, int s, int32_t* cell_count_out
         c->launches++;
     }
     sp.state = ST_SEGMENTED;
+    sp.nearly_sorted = true;
     sp.leavers_pending = false;
     return ECSIM_OK;
 }

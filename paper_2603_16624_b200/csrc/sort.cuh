@@ -148,3 +148,106 @@ k_copy_u32_to_i32(uint32_t m, const uint32_t* __restrict__ in, int32_t* __restri
     for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < m; p += stride)
         out[p] = (int32_t)in[p];
 }
+
+// ---------------------------------------------------------------------------------------------
+// Moving the seven SoA arrays of a species given in RANDOM order (config 4) to their sorted places.
+// A random 8-byte gather from HBM costs ~97 bytes of traffic on B200 (3.26 GB per 33.5 M elements,
+// profiles/r01d), and scattered 8-byte stores are bound by L2 transactions, so the permutation is applied in
+// two steps that are both local.  dest[p] = start[cell[p]] + rank[p] is the final place of particle p;
+// places are cut into <= SORT_MAX_BUCKETS buckets of 2^shift consecutive places (every bucket is full,
+// dest being a permutation).
+//   step A, k_stage_to_slots: a tile of SORT_TILE particles per CTA.  slot[p] = (places of p's bucket taken by
+//          earlier tiles) + (p's arrival rank in the tile).  The tile is ordered by bucket in shared memory and
+//          written to tmp[] in runs of ~SORT_TILE/buckets consecutive elements: coalesced.
+//   step B, k_gather_f64 with perm2[dest[p]] = slot[p]: out[d] = tmp[perm2[d]], a gather whose sources lie
+//          inside one bucket's window of tmp (<= 1 MB): L2 hits; the writes are coalesced.
+// slot and perm2 are computed once and serve all seven arrays; tmp is the one spare array and `out` is the
+// caller's own array, so nothing is copied back.  (A species that is re-sorted after a push is nearly
+// sorted: there the direct gather of ecsim_sort_particles reads almost sequentially and stays.)
+constexpr int SORT_TILE = 8192;
+constexpr int SORT_MAX_BUCKETS = 512;
+constexpr int SORT_STAGE_THREADS = 512;
+constexpr size_t SORT_STAGE_SMEM = (size_t)SORT_TILE * (sizeof(double) + sizeof(uint32_t)) + 2 * SORT_MAX_BUCKETS * sizeof(uint32_t);
+
+// dest (in place of rank) and the per-(bucket, tile) histogram H[b * tiles + tile]
+__global__ void __launch_bounds__(256)
+k_dest_and_tile_hist(uint32_t n, const int32_t* __restrict__ cell, uint32_t* __restrict__ rank_to_dest,
+                     const uint32_t* __restrict__ start, int shift, uint32_t tiles, uint32_t* __restrict__ H)
+{
+    __shared__ uint32_t cnt[SORT_MAX_BUCKETS];
+    for (int t = threadIdx.x; t < SORT_MAX_BUCKETS; t += blockDim.x) cnt[t] = 0;
+    __syncthreads();
+    const size_t p0 = (size_t)blockIdx.x * SORT_TILE;
+    for (int e = threadIdx.x; e < SORT_TILE; e += blockDim.x) {
+        const size_t p = p0 + e;
+        if (p < n) {
+            const uint32_t d = start[cell[p]] + rank_to_dest[p];
+            rank_to_dest[p] = d;
+            atomicAdd(&cnt[d >> shift], 1u);
+        }
+    }
+    __syncthreads();
+    const uint32_t nb = ((n - 1) >> shift) + 1;
+    for (uint32_t b = threadIdx.x; b < nb; b += blockDim.x) H[(size_t)b * tiles + blockIdx.x] = cnt[b];
+}
+
+// slot[p] (over the cell array's storage) and perm2[dest[p]] = slot[p]; Hs = exclusive scan of H
+__global__ void __launch_bounds__(256)
+k_assign_slots(uint32_t n, const uint32_t* __restrict__ dest, const uint32_t* __restrict__ Hs, int shift,
+               uint32_t tiles, uint32_t* __restrict__ slot, uint32_t* __restrict__ perm2)
+{
+    __shared__ uint32_t base[SORT_MAX_BUCKETS];
+    const uint32_t nb = ((n - 1) >> shift) + 1;
+    for (uint32_t b = threadIdx.x; b < nb; b += blockDim.x) base[b] = Hs[(size_t)b * tiles + blockIdx.x];
+    __syncthreads();
+    const size_t p0 = (size_t)blockIdx.x * SORT_TILE;
+    for (int e = threadIdx.x; e < SORT_TILE; e += blockDim.x) {
+        const size_t p = p0 + e;
+        if (p < n) {
+            const uint32_t d = dest[p];
+            const uint32_t s = atomicAdd(&base[d >> shift], 1u);
+            slot[p] = s;
+            perm2[d] = s;
+        }
+    }
+}
+
+// step A for one array: tmp[slot[p]] = in[p], the tile ordered by bucket in shared memory first
+__global__ void __launch_bounds__(SORT_STAGE_THREADS)
+k_stage_to_slots(uint32_t n, const uint32_t* __restrict__ dest, const uint32_t* __restrict__ slot,
+                 const uint32_t* __restrict__ H, const uint32_t* __restrict__ Hs, int shift, uint32_t tiles,
+                 const double* __restrict__ in, double* __restrict__ tmp)
+{
+    extern __shared__ __align__(16) unsigned char stage_smem[];
+    double* vals = reinterpret_cast<double*>(stage_smem);
+    uint32_t* dsts = reinterpret_cast<uint32_t*>(vals + SORT_TILE);
+    uint32_t* base = dsts + SORT_TILE;          // first slot of this tile's share of bucket b
+    uint32_t* toff = base + SORT_MAX_BUCKETS;   // where bucket b starts in the tile's bucket order
+    __shared__ uint32_t total;
+    const uint32_t nb = ((n - 1) >> shift) + 1;
+    const uint32_t b = threadIdx.x;
+    const uint32_t c = b < nb ? H[(size_t)b * tiles + blockIdx.x] : 0u;
+    const uint32_t ex = block_exclusive_scan(c, &total);
+    toff[b] = ex;
+    base[b] = b < nb ? Hs[(size_t)b * tiles + blockIdx.x] : 0u;
+    __syncthreads();
+    const size_t p0 = (size_t)blockIdx.x * SORT_TILE;
+    const uint32_t tile_n = (uint32_t)min((size_t)SORT_TILE, (size_t)n - p0);
+    for (uint32_t e = threadIdx.x; e < tile_n; e += SORT_STAGE_THREADS) {
+        const size_t p = p0 + e;
+        const uint32_t s = slot[p], bk = dest[p] >> shift;
+        const uint32_t lp = s - base[bk] + toff[bk];
+        vals[lp] = in[p];
+        dsts[lp] = s;
+    }
+    __syncthreads();
+    for (uint32_t t = threadIdx.x; t < tile_n; t += SORT_STAGE_THREADS) tmp[dsts[t]] = vals[t];
+}
+
+// perm[dest[p]] = p (only when the caller asks for the permutation)
+__global__ void __launch_bounds__(256)
+k_perm_from_dest(uint32_t n, const uint32_t* __restrict__ dest, uint32_t* __restrict__ perm)
+{
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += stride) perm[dest[p]] = (uint32_t)p;
+}
