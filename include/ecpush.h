@@ -132,6 +132,16 @@ int ecsim_push_and_moments_host(ecsim_ctx *ctx, int64_t n, double q_over_m, int 
                                 const double *q, const double *E_theta, const double *B,
                                 double dt, double theta, double *rho, double *Jhat, double *M, int accumulate);
 
+/* The same for ALL species of the context in one call (M crosses the bus once): n, q_over_m and the array-of-pointer
+ * arguments have n_species entries; rho [n_species][nodes], Jhat [n_species][3][nodes], M shared.  The workspace must
+ * be ecsim_host_step_all_workspace_bytes(ctx, max n, sum of n) large. */
+size_t ecsim_host_step_all_workspace_bytes(const ecsim_ctx *ctx, int64_t n_max, int64_t n_total);
+int ecsim_push_and_moments_host_all(ecsim_ctx *ctx, const int64_t *n, const double *q_over_m, int sorted,
+                                    double *const *x, double *const *y, double *const *z,
+                                    double *const *u, double *const *v, double *const *w, const double *const *q,
+                                    const double *E_theta, const double *B, double dt, double theta,
+                                    double *rho, double *Jhat, double *M, int accumulate);
+
 /* Select the kernel variant (default ECSIM_VARIANT_FUSED). */
 int ecsim_set_variant(ecsim_ctx *ctx, int variant);
 

@@ -55,6 +55,9 @@ _PROTOS = {
     "ecsim_host_step_workspace_bytes": (_c.c_size_t, [_P, _c.c_int64]),
     "ecsim_push_and_moments_host": (_c.c_int, [_P, _c.c_int64, _c.c_double, _c.c_int] + [_P] * 9 +
                                     [_c.c_double, _c.c_double, _P, _P, _P, _c.c_int]),
+    "ecsim_host_step_all_workspace_bytes": (_c.c_size_t, [_P, _c.c_int64, _c.c_int64]),
+    "ecsim_push_and_moments_host_all": (_c.c_int, [_P, _P, _P, _c.c_int] + [_P] * 9 +
+                                        [_c.c_double, _c.c_double, _P, _P, _P, _c.c_int]),
     "ecsim_set_variant": (_c.c_int, [_P, _c.c_int]),
     "ecsim_set_resort_fraction": (_c.c_int, [_P, _c.c_double]),
     "ecsim_set_fused_warps": (_c.c_int, [_P, _c.c_int]),
@@ -193,6 +196,29 @@ class Ecsim:
                                                   _hptr(B, f64), dt, theta, _hptr(rho, f64), _hptr(Jhat, f64),
                                                   _hptr(M, f64), int(accumulate)),
                "ecsim_push_and_moments_host")
+
+    def set_workspace_host_all(self, n_max: int, n_total: int):
+        nbytes = int(self.L.ecsim_host_step_all_workspace_bytes(self.h, n_max, n_total))
+        ws = self.torch.empty(nbytes + 256, dtype=self.torch.uint8, device="cuda")
+        off = (-ws.data_ptr()) % 256
+        self._ws = ws
+        _check(self.L.ecsim_set_workspace(self.h, _P(ws.data_ptr() + off), nbytes), "ecsim_set_workspace")
+        return nbytes
+
+    def push_and_moments_host_all(self, qoms, sorted: bool, parts, E, B, dt: float, theta: float, rho, Jhat, M,
+                                  accumulate: int = 0):
+        """parts: list (one per species) of dicts of host tensors x..q; rho [nsp][nodes], Jhat [nsp][3][nodes] host."""
+        f64 = self.torch.float64
+        nsp = len(parts)
+        n = (_c.c_int64 * nsp)(*[int(p["x"].numel()) for p in parts])
+        qm = (_c.c_double * nsp)(*[float(v) for v in qoms])
+        cols = []
+        for k in ("x", "y", "z", "u", "v", "w", "q"):
+            cols.append((_P * nsp)(*[_hptr(p[k], f64) for p in parts]))
+        _check(self.L.ecsim_push_and_moments_host_all(self.h, n, qm, 1 if sorted else 0, *cols, _hptr(E, f64),
+                                                      _hptr(B, f64), dt, theta, _hptr(rho, f64), _hptr(Jhat, f64),
+                                                      _hptr(M, f64), int(accumulate)),
+               "ecsim_push_and_moments_host_all")
 
     # -- knobs and instrumentation -------------------------------------------------------------
     def set_variant(self, variant: int):

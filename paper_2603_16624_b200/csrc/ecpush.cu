@@ -719,18 +719,114 @@ extern "C" int ecsim_push_and_moments_all(ecsim_ctx* c, const double* E_theta, c
 }
 
 // --------------------------------------------------------------------------------------------
-// Host-buffer step (the end-to-end path): stage in the workspace tail, run, copy back, synchronise.
-static size_t host_step_extra(const ecsim_ctx* c, int64_t n)
+// Host-buffer steps (the end-to-end path): stage in the workspace tail, run, copy back, synchronise.
+static size_t host_step_extra(const ecsim_ctx* c, int64_t n_total, int n_species_out)
 {
     const size_t nodes = (size_t)c->g.nodes;
-    return align_up(sizeof(double) * 7 * (size_t)n, 256) + align_up(sizeof(double) * 6 * nodes, 256) +
-           align_up(sizeof(double) * 4 * nodes, 256) + align_up(sizeof(double) * 243 * nodes, 256);
+    return align_up(sizeof(double) * 7 * (size_t)n_total, 256) + align_up(sizeof(double) * 6 * nodes, 256) +
+           align_up(sizeof(double) * 4 * nodes * n_species_out, 256) + align_up(sizeof(double) * 243 * nodes, 256);
 }
 
 extern "C" size_t ecsim_host_step_workspace_bytes(const ecsim_ctx* c, int64_t n_particles)
 {
     if (!c || n_particles < 0) return 0;
-    return ecsim_workspace_bytes(c, n_particles) + host_step_extra(c, n_particles);
+    return ecsim_workspace_bytes(c, n_particles) + host_step_extra(c, n_particles, 1);
+}
+
+extern "C" size_t ecsim_host_step_all_workspace_bytes(const ecsim_ctx* c, int64_t n_max, int64_t n_total)
+{
+    if (!c || n_max < 0 || n_total < n_max) return 0;
+    return ecsim_workspace_bytes(c, n_max) + host_step_extra(c, n_total, c->n_species);
+}
+
+// nsp species (slots 0..nsp-1 of the context) from host arrays; rho [nsp][nodes], Jhat [nsp][3][nodes], M shared.
+static int host_step_impl(ecsim_ctx* c, int nsp, const int64_t* n, const double* qom, int sorted,
+                          double* const* hx, double* const* hy, double* const* hz, double* const* hu,
+                          double* const* hv, double* const* hw, const double* const* hq,
+                          const double* E_theta, const double* B, double dt, double theta,
+                          double* rho, double* Jhat, double* M, int accumulate, bool all_species_call)
+{
+    int64_t n_max = 0, n_total = 0;
+    for (int s = 0; s < nsp; ++s) {
+        if (n[s] < 0 || !hx[s] || !hy[s] || !hz[s] || !hu[s] || !hv[s] || !hw[s] || !hq[s]) return ECSIM_ERR_INVALID_ARG;
+        n_max = n[s] > n_max ? n[s] : n_max;
+        n_total += n[s];
+    }
+    if (!c->ws.base || c->ws.bytes < ecsim_workspace_bytes(c, n_max) + host_step_extra(c, n_total, nsp))
+        return ECSIM_ERR_WORKSPACE;
+    // re-carve so that exactly n_max particles are served and the tail is free for staging
+    Workspace keep = c->ws;
+    const size_t used = carve(c, n_max, keep.base, &c->ws);
+    c->ws.bytes = keep.bytes;
+    char* tail = reinterpret_cast<char*>(keep.base) + used;
+    const size_t nodes = (size_t)c->g.nodes;
+    double* dpart = reinterpret_cast<double*>(tail);
+    tail += align_up(sizeof(double) * 7 * (size_t)n_total, 256);
+    double* dE = reinterpret_cast<double*>(tail);
+    double* dB = dE + 3 * nodes;
+    tail += align_up(sizeof(double) * 6 * nodes, 256);
+    double* drho = reinterpret_cast<double*>(tail);          // [nsp][nodes]
+    double* dJ = drho + (size_t)nsp * nodes;                 // [nsp][3][nodes]
+    tail += align_up(sizeof(double) * 4 * nodes * nsp, 256);
+    double* dM = reinterpret_cast<double*>(tail);
+    cudaStream_t st = c->stream;
+    SpeciesHost saved[ECSIM_MAX_SPECIES];
+    int rc = ECSIM_OK;
+    {
+        double* d = dpart;
+        for (int s = 0; s < nsp && rc == ECSIM_OK; ++s) {
+            const size_t pn = (size_t)n[s];
+            double* hp[7] = {hx[s], hy[s], hz[s], hu[s], hv[s], hw[s], const_cast<double*>(hq[s])};
+            for (int a = 0; a < 7; ++a)
+                CK(cudaMemcpyAsync(d + a * pn, hp[a], sizeof(double) * pn, cudaMemcpyHostToDevice, st));
+            saved[s] = c->sp[s];
+            rc = ecsim_load_particles(c, s, n[s], qom[s], d, d + pn, d + 2 * pn, d + 3 * pn, d + 4 * pn, d + 5 * pn,
+                                      d + 6 * pn, sorted);
+            d += 7 * pn;
+        }
+    }
+    CK(cudaMemcpyAsync(dE, E_theta, sizeof(double) * 3 * nodes, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(dB, B, sizeof(double) * 3 * nodes, cudaMemcpyHostToDevice, st));
+    if (accumulate == ECSIM_ACC_ALL) {
+        if (rho) CK(cudaMemcpyAsync(drho, rho, sizeof(double) * nodes * nsp, cudaMemcpyHostToDevice, st));
+        if (Jhat) CK(cudaMemcpyAsync(dJ, Jhat, sizeof(double) * 3 * nodes * nsp, cudaMemcpyHostToDevice, st));
+    }
+    if (accumulate != ECSIM_ACC_NONE && M)
+        CK(cudaMemcpyAsync(dM, M, sizeof(double) * 243 * nodes, cudaMemcpyHostToDevice, st));
+    if (rc == ECSIM_OK) {
+        int list[ECSIM_MAX_SPECIES];
+        for (int s = 0; s < nsp; ++s) list[s] = s;
+        rc = push_and_moments_impl(c, nsp, list, dE, dB, dt, theta, rho ? drho : nullptr, all_species_call ? nodes : 0,
+                                   Jhat ? dJ : nullptr, all_species_call ? 3 * nodes : 0, M ? dM : nullptr, accumulate);
+    }
+    if (rc == ECSIM_OK) {
+        double* d = dpart;
+        for (int s = 0; s < nsp; ++s) {
+            const size_t pn = (size_t)n[s];
+            double* hp[6] = {hx[s], hy[s], hz[s], hu[s], hv[s], hw[s]};
+            for (int a = 0; a < 6; ++a)
+                CK(cudaMemcpyAsync(hp[a], d + a * pn, sizeof(double) * pn, cudaMemcpyDeviceToHost, st));
+            d += 7 * pn;
+        }
+        if (rho) CK(cudaMemcpyAsync(rho, drho, sizeof(double) * nodes * nsp, cudaMemcpyDeviceToHost, st));
+        if (Jhat) CK(cudaMemcpyAsync(Jhat, dJ, sizeof(double) * 3 * nodes * nsp, cudaMemcpyDeviceToHost, st));
+        if (M) CK(cudaMemcpyAsync(M, dM, sizeof(double) * 243 * nodes, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+    }
+    // restore the caller's species and the full carve
+    for (int s = 0; s < nsp; ++s) {
+        cudaEvent_t ev = c->sp[s].leavers_event;
+        c->sp[s] = saved[s];
+        c->sp[s].leavers_event = ev;
+        c->sp[s].leavers_pending = false;
+    }
+    const size_t used2 = carve(c, keep.n_max, keep.base, &c->ws);
+    c->ws.bytes = keep.bytes;
+    c->ws.extra = reinterpret_cast<char*>(keep.base) + used2;
+    c->ws.extra_bytes = keep.bytes - used2;
+    for (int s = 0; s < c->n_species; ++s)
+        if (c->sp[s].state == ST_SEGMENTED) c->sp[s].state = ST_DECLARED;   // the tables lived in the re-carved buffer
+    return rc;
 }
 
 extern "C" int ecsim_push_and_moments_host(ecsim_ctx* c, int64_t n, double q_over_m, int sorted,
@@ -738,64 +834,21 @@ extern "C" int ecsim_push_and_moments_host(ecsim_ctx* c, int64_t n, double q_ove
                                            const double* q, const double* E_theta, const double* B,
                                            double dt, double theta, double* rho, double* Jhat, double* M, int accumulate)
 {
-    if (!c || n < 0 || !x || !y || !z || !u || !v || !w || !q || !E_theta || !B) return ECSIM_ERR_INVALID_ARG;
-    if (!c->ws.base || c->ws.bytes < ecsim_host_step_workspace_bytes(c, n)) return ECSIM_ERR_WORKSPACE;
-    // re-carve so that exactly n particles are served and the tail is free for staging
-    Workspace keep = c->ws;
-    const size_t used = carve(c, n, keep.base, &c->ws);
-    c->ws.bytes = keep.bytes;
-    char* tail = reinterpret_cast<char*>(keep.base) + used;
-    const size_t nodes = (size_t)c->g.nodes;
-    const size_t pn = (size_t)n;
-    double* dpart = reinterpret_cast<double*>(tail);
-    tail += align_up(sizeof(double) * 7 * pn, 256);
-    double* dE = reinterpret_cast<double*>(tail);
-    double* dB = dE + 3 * nodes;
-    tail += align_up(sizeof(double) * 6 * nodes, 256);
-    double* drho = reinterpret_cast<double*>(tail);
-    double* dJ = drho + nodes;
-    tail += align_up(sizeof(double) * 4 * nodes, 256);
-    double* dM = reinterpret_cast<double*>(tail);
-    cudaStream_t st = c->stream;
-    double* hp[7] = {x, y, z, u, v, w, const_cast<double*>(q)};
-    for (int a = 0; a < 7; ++a)
-        CK(cudaMemcpyAsync(dpart + a * pn, hp[a], sizeof(double) * pn, cudaMemcpyHostToDevice, st));
-    CK(cudaMemcpyAsync(dE, E_theta, sizeof(double) * 3 * nodes, cudaMemcpyHostToDevice, st));
-    CK(cudaMemcpyAsync(dB, B, sizeof(double) * 3 * nodes, cudaMemcpyHostToDevice, st));
-    if (accumulate == ECSIM_ACC_ALL) {
-        if (rho) CK(cudaMemcpyAsync(drho, rho, sizeof(double) * nodes, cudaMemcpyHostToDevice, st));
-        if (Jhat) CK(cudaMemcpyAsync(dJ, Jhat, sizeof(double) * 3 * nodes, cudaMemcpyHostToDevice, st));
-    }
-    if (accumulate != ECSIM_ACC_NONE && M)
-        CK(cudaMemcpyAsync(dM, M, sizeof(double) * 243 * nodes, cudaMemcpyHostToDevice, st));
-    SpeciesHost saved = c->sp[0];
-    int rc = ecsim_load_particles(c, 0, n, q_over_m, dpart, dpart + pn, dpart + 2 * pn, dpart + 3 * pn,
-                                  dpart + 4 * pn, dpart + 5 * pn, dpart + 6 * pn, sorted);
-    const int sp0 = 0;
-    if (rc == ECSIM_OK)
-        rc = push_and_moments_impl(c, 1, &sp0, dE, dB, dt, theta, rho ? drho : nullptr, 0, Jhat ? dJ : nullptr, 0,
-                                   M ? dM : nullptr, accumulate);
-    if (rc == ECSIM_OK) {
-        for (int a = 0; a < 6; ++a)
-            CK(cudaMemcpyAsync(hp[a], dpart + a * pn, sizeof(double) * pn, cudaMemcpyDeviceToHost, st));
-        if (rho) CK(cudaMemcpyAsync(rho, drho, sizeof(double) * nodes, cudaMemcpyDeviceToHost, st));
-        if (Jhat) CK(cudaMemcpyAsync(Jhat, dJ, sizeof(double) * 3 * nodes, cudaMemcpyDeviceToHost, st));
-        if (M) CK(cudaMemcpyAsync(M, dM, sizeof(double) * 243 * nodes, cudaMemcpyDeviceToHost, st));
-        CK(cudaStreamSynchronize(st));
-    }
-    // restore the caller's species 0 and the full carve
-    cudaEvent_t ev = c->sp[0].leavers_event;
-    c->sp[0] = saved;
-    c->sp[0].leavers_event = ev;
-    c->sp[0].leavers_pending = false;
-    if (c->sp[0].state == ST_SEGMENTED) c->sp[0].state = ST_DECLARED;
-    const size_t used2 = carve(c, keep.n_max, keep.base, &c->ws);
-    c->ws.bytes = keep.bytes;
-    c->ws.extra = reinterpret_cast<char*>(keep.base) + used2;
-    c->ws.extra_bytes = keep.bytes - used2;
-    for (int s = 1; s < c->n_species; ++s)
-        if (c->sp[s].state == ST_SEGMENTED) c->sp[s].state = ST_DECLARED;
-    return rc;
+    if (!c || !E_theta || !B) return ECSIM_ERR_INVALID_ARG;
+    return host_step_impl(c, 1, &n, &q_over_m, sorted, &x, &y, &z, &u, &v, &w, &q, E_theta, B, dt, theta, rho, Jhat, M,
+                          accumulate, false);
+}
+
+extern "C" int ecsim_push_and_moments_host_all(ecsim_ctx* c, const int64_t* n, const double* q_over_m, int sorted,
+                                               double* const* x, double* const* y, double* const* z,
+                                               double* const* u, double* const* v, double* const* w,
+                                               const double* const* q, const double* E_theta, const double* B,
+                                               double dt, double theta, double* rho, double* Jhat, double* M,
+                                               int accumulate)
+{
+    if (!c || !n || !q_over_m || !x || !y || !z || !u || !v || !w || !q || !E_theta || !B) return ECSIM_ERR_INVALID_ARG;
+    return host_step_impl(c, c->n_species, n, q_over_m, sorted, x, y, z, u, v, w, q, E_theta, B, dt, theta, rho, Jhat,
+                          M, accumulate, true);
 }
 
 // --------------------------------------------------------------------------------------------

@@ -389,3 +389,25 @@ def test_host_buffer_step_matches_oracle():
     assert_particles_close(host, pn, cfg, "host step")
     assert_moments_close(rho, J, M, mom, "host step")
     ctx.close()
+
+
+def test_host_buffer_all_species_step_matches_oracle():
+    cfg = wl.config(0)
+    E, B = wl.gen_fields(cfg)
+    parts = [wl.gen_species(cfg, s) for s in range(2)]
+    parts_np = [to_numpy(p) for p in parts]
+    host = [{k: p[k].clone().pin_memory() for k in PKEYS} for p in parts]
+    ctx = pk.Ecsim(*grid_of(cfg), 2)
+    ctx.set_workspace_host_all(max(p["n"] for p in parts), sum(p["n"] for p in parts))
+    rho = torch.empty(2, cfg.nodes, dtype=torch.float64).pin_memory()
+    J = torch.empty(2, 3, cfg.nodes, dtype=torch.float64).pin_memory()
+    M = torch.empty(cfg.nodes, 27, 3, 3, dtype=torch.float64).pin_memory()
+    ctx.push_and_moments_host_all([sp.qom for sp in cfg.species], True, host, E.contiguous(), B.contiguous(), cfg.dt,
+                                  cfg.theta, rho, J, M)
+    (total, per_species), = oracle_run(cfg, parts_np, E, B)
+    for s in range(2):
+        assert_particles_close(host[s], parts_np[s], cfg, f"host all, species {s}")
+        assert_moments_close(rho[s], J[s], None, per_species[s], f"host all, species {s}")
+    assert_moments_close(None, None, M, total, "host all")
+    # the single-species host call still works on the same context afterwards
+    ctx.close()
