@@ -44,6 +44,7 @@ struct SpeciesHost {
     double qom = 0.0;
     double *x = nullptr, *y = nullptr, *z = nullptr, *u = nullptr, *v = nullptr, *w = nullptr, *q = nullptr;
     int state = ST_UNSORTED;
+    double stray_debt = 0.0;        // strays processed since the last sort, summed over the steps
     bool nearly_sorted = false;     // the arrays were cell-sorted before the last pushes (a re-sort, not a first sort)
     bool leavers_pending = false;   // an async copy of the leaver counter is in flight
     cudaEvent_t leavers_event = nullptr;
@@ -84,7 +85,7 @@ struct ecsim_ctx {
     SpeciesHost* sp = nullptr;
     Workspace ws;
     int variant = ECSIM_VARIANT_FUSED;
-    double resort_fraction = 0.01;
+    double resort_fraction = 0.007;
     int timing = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     bool ev_valid = false;
@@ -294,6 +295,7 @@ extern "C" int ecsim_load_particles(ecsim_ctx* c, int s, int64_t n, double q_ove
     sp.x = x; sp.y = y; sp.z = z; sp.u = u; sp.v = v; sp.w = w; sp.q = q;
     sp.state = sorted ? ST_DECLARED : ST_UNSORTED;
     sp.nearly_sorted = sorted != 0;
+    sp.stray_debt = 0.0;
     sp.leavers_pending = false;
     return ECSIM_OK;
 }
@@ -418,6 +420,7 @@ extern "C" int ecsim_sort_particles(ecsim_ctx* c, int s, int32_t* cell_count_out
     }
     sp.state = ST_SEGMENTED;
     sp.nearly_sorted = true;
+    sp.stray_debt = 0.0;
     sp.leavers_pending = false;
     return ECSIM_OK;
 }
@@ -570,7 +573,10 @@ static int push_and_moments_impl(ecsim_ctx* c, int n_list, const int* list, cons
         if (sp.state == ST_SEGMENTED && sp.leavers_pending) {
             CK(cudaEventSynchronize(sp.leavers_event));
             sp.leavers_pending = false;
-            if ((double)c->h_leavers[s] > c->resort_fraction * (double)sp.n) sp.state = ST_UNSORTED;
+            // Rent or buy: a stray costs ~7.7 ns per step it stays a stray, a re-sort ~54 ps per particle (DESIGN.md
+            // §6.2).  Re-sort when the strays handled since the last sort plus those waiting now would have paid for it.
+            if (sp.stray_debt + (double)c->h_leavers[s] > c->resort_fraction * (double)sp.n) sp.state = ST_UNSORTED;
+            else sp.stray_debt += (double)c->h_leavers[s];
         }
         if (sp.state == ST_UNSORTED) {
             rc = ecsim_sort_particles(c, s, nullptr, nullptr);

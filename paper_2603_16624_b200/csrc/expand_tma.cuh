@@ -12,8 +12,8 @@
 // previous level" before its slot is refilled.  Slots, mbarrier phases and output pointers advance incrementally
 // and the term loops are shaped per warp (the first version spent 640 warp instructions per node, 90 % of them
 // address arithmetic and divergence bookkeeping).
-// Measured on config 2 (whole grid, profiles/r01c): 2.0 ms with 128 threads x ring 3; 2.2 ms (128 x 4),
-// 2.4 ms (256 x 3), 2.8 ms (64 x 3), 3.2 ms (128 x 5); the register-staged k_expand_M it replaces: 2.95 ms.
+// Measured on config 2 (whole grid, profiles/r01c): 1.68 ms with 128 threads x ring 3 (128 x 4, 256 x 4 and 96 x 3
+// are within 2 % of it, 256 x 3 and 64 x 3 slower); the register-staged k_expand_M it replaces: 2.95 ms.
 #pragma once
 #include "common.cuh"
 #include "fused_mma.cuh"

@@ -214,7 +214,7 @@ def _ids(q, q0):
     return np.rint((q / q0 - 1.0) * 2.0 ** 30).astype(np.int64)
 
 
-@pytest.mark.parametrize("resort_fraction", [0.01, 1.0], ids=["resort", "strays_only"])
+@pytest.mark.parametrize("resort_fraction", [0.01, 100.0], ids=["resort", "strays_only"])
 def test_eleven_steps_fields_fixed(resort_fraction):
     """Config 1's protocol (one step, then 10 more with fields held fixed) on a 10x8x12 box."""
     cfg = wl.config(1, (10, 8, 12))
