@@ -110,8 +110,8 @@ int ecsim_cell_index(ecsim_ctx *ctx, int species, int32_t *cell_out);
  * With variant FUSED an unsorted species is sorted first (same effect as ecsim_sort_particles).  After the
  * call the species keeps its segment table; the kernel counts the particles that left their cell, and the
  * next call re-sorts first when that count, plus the strays handled since the last sort, exceeds
- * ecsim_set_resort_fraction() * n (default 0.7 %: the measured cost of a re-sort in strays), otherwise
- * the leavers are handled as strays (pushed one thread per particle, deposited with atomics into the per-cell
+ * ecsim_set_resort_fraction() * n (default 4 %: the measured cost of a re-sort in strays), otherwise
+ * the leavers are handled as strays (pushed one warp per particle, added with one bulk reduction to the per-cell
  * accumulators of their true cell before the expansion).  (The count is read through pinned memory: the next
  * call waits for this call's kernels to finish before it decides.) */
 int ecsim_push_and_moments(ecsim_ctx *ctx, int species, const double *E_theta, const double *B,
@@ -147,7 +147,7 @@ int ecsim_push_and_moments_host_all(ecsim_ctx *ctx, const int64_t *n, const doub
 int ecsim_set_variant(ecsim_ctx *ctx, int variant);
 
 /* Tuning knobs: fraction of a species that may sit outside its cell segment before the next step re-sorts
- * (default 0.007); warps per CTA of the fused kernel (8, 12 or 16, with 224, 168 or 128 registers per thread;
+ * (default 0.04); warps per CTA of the fused kernel (8, 12 or 16, with 224, 168 or 128 registers per thread;
  * default 12; always 12 x 144 when slabs overlap). */
 int ecsim_set_resort_fraction(ecsim_ctx *ctx, double fraction);
 int ecsim_set_fused_warps(ecsim_ctx *ctx, int warps);

@@ -133,11 +133,11 @@ k_push_moments_atomic(AtomicArgs a)
 }
 
 // ---------------------------------------------------------------------------------------------
-// Strays of the fused variant, deposited into the PER-CELL accumulators of their true cell instead of the
-// node arrays: AM[cell][class][ij] and AJ[cell][corner][4] (layouts of fused_mma.cuh), after the fused kernel
-// stored them and before the expansion reads them.  A stray then costs 243 + 32 atomics on one contiguous
-// 2.2 KB block instead of 576 + 32 atomics spread over 8 node blocks of 1.9 KB each (16 KB of HBM
-// read-modify-write per stray: measured 16 ns per stray, profiles/r01d).  Push as in k_push_moments_atomic.
+// Strays of the fused variant are deposited into the PER-CELL accumulators of their true cell -- AM[cell][class][ij]
+// and AJ[cell][corner][4] (layouts of fused_mma.cuh) -- after the fused kernel stored them and before the expansion
+// reads them.  Cost per stray, measured on config 2 (profiles/r01d): 16 ns with 576 + 32 atomics on the node arrays
+// (eight 1.9 KB node blocks of HBM read-modify-write), 7.7 ns with 243 + 32 atomics on the cell's block, 1.4-2.2 ns
+// with the bulk reduction below.
 struct StrayArgs {
     Geom g;
     const uint32_t* list;       // indices of the strays
@@ -151,14 +151,36 @@ struct StrayArgs {
     unsigned long long* leavers;
 };
 
-__global__ void __launch_bounds__(128)
-k_push_strays_to_cells(StrayArgs a, int am_per_cell, int am_a8)
+// ---------------------------------------------------------------------------------------------
+// ONE bulk reduction per stray instead of 275 atomics: a warp handles a stray, builds its
+// 244-double contribution to AM[cell] (and 32 doubles to AJ[cell]) in shared memory -- lane = class for the mass
+// matrix, lane = corner for rho / Jhat -- and adds both blocks to global memory with cp.reduce.async.bulk
+// (.add.f64: the reduction runs in L2 on whole sectors; SASS UBLKRED).  All lanes compute the particle's scalars
+// redundantly; lane 0 writes the pushed particle back.
+constexpr int STRAY_WARPS = 4;
+constexpr int STRAY_SMEM_DOUBLES = 244 + 32;
+
+__device__ __forceinline__ void bulk_reduce_add_f64(double* dst_global, const double* src_shared, unsigned bytes)
 {
+    asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.f64 [%0], [%1], %2;"
+                 ::"l"(dst_global), "r"((uint32_t)__cvta_generic_to_shared(src_shared)), "r"(bytes) : "memory");
+}
+
+__global__ void __launch_bounds__(STRAY_WARPS * 32)
+k_push_strays_bulk(StrayArgs a, int am_per_cell, int am_a8)
+{
+    __shared__ __align__(128) double stage[STRAY_WARPS][STRAY_SMEM_DOUBLES];
     const Geom& g = a.g;
-    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double* sm = stage[warp];
     const size_t count = (size_t)*a.list_count;
+    const size_t wstride = (size_t)gridDim.x * STRAY_WARPS;
     unsigned my_leavers = 0;
-    for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < count; t += stride) {
+    // lane roles: class (kx, ky, kz) of lanes 0..26; corner (ca, cb, cc) of lanes 0..7
+    const int cls = lane < 27 ? lane : 0;
+    const int kx = cls / 9, ky = (cls / 3) % 3, kz = cls % 3;
+    const int ca = (lane >> 2) & 1, cb = (lane >> 1) & 1, cc = lane & 1;
+    for (size_t t = (size_t)blockIdx.x * STRAY_WARPS + warp; t < count; t += wstride) {
         const size_t p = a.list[t];
         const double x = a.x[p], y = a.y[p], z = a.z[p];
         const double vx = a.u[p], vy = a.v[p], vz = a.w[p];
@@ -170,16 +192,16 @@ k_push_strays_to_cells(StrayArgs a, int am_per_cell, int am_a8)
         const int k1 = (k0 + 1 == g.nz) ? 0 : k0 + 1;
         const double xi = sx - i0, eta = sy - j0, zeta = sz - k0;
         const double wx[2] = {1.0 - xi, xi}, wy[2] = {1.0 - eta, eta}, wz[2] = {1.0 - zeta, zeta};
-        double W[8], Ep[3] = {0, 0, 0}, Bp[3] = {0, 0, 0};
+        double Ep[3] = {0, 0, 0}, Bp[3] = {0, 0, 0};
 #pragma unroll
         for (int c = 0; c < 8; ++c) {
             const int ia = (c >> 2) & 1, ib = (c >> 1) & 1, ic = c & 1;
-            W[c] = (wx[ia] * wy[ib]) * wz[ic];
+            const double Wc = (wx[ia] * wy[ib]) * wz[ic];
             const long long node = ((long long)(ia ? i1 : i0) * g.ny + (ib ? j1 : j0)) * g.nz + (ic ? k1 : k0);
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
-                Ep[d] += W[c] * __ldg(a.E + d * g.nodes + node);
-                Bp[d] += W[c] * __ldg(a.B + d * g.nodes + node);
+                Ep[d] += Wc * __ldg(a.E + d * g.nodes + node);
+                Bp[d] += Wc * __ldg(a.B + d * g.nodes + node);
             }
         }
         // rotation matrix, Eq. (2) as nine scalars (L53, L135); (I x B) v = B x v
@@ -192,42 +214,45 @@ k_push_strays_to_cells(StrayArgs a, int am_per_cell, int am_a8)
         const double vh[3] = {al[0] * vx + al[1] * vy + al[2] * vz, al[3] * vx + al[4] * vy + al[5] * vz,
                               al[6] * vx + al[7] * vy + al[8] * vz};
         const double qV = q * g.invV, qbV = qV * a.beta;
+        // this lane's class weight: p?[0..2] = (w0^2, w0 w1, w1^2) per axis (Eq. 3)
+        const double fx = (kx == 0 ? wx[0] * wx[0] : kx == 1 ? wx[0] * wx[1] : wx[1] * wx[1]);
+        const double fy = (ky == 0 ? wy[0] * wy[0] : ky == 1 ? wy[0] * wy[1] : wy[1] * wy[1]);
+        const double fz = (kz == 0 ? wz[0] * wz[0] : kz == 1 ? wz[0] * wz[1] : wz[1] * wz[1]);
+        const double cf = qbV * ((fx * fy) * fz);
+        if (lane < 27) {
+#pragma unroll
+            for (int e = 0; e < 8; e += 2)
+                *reinterpret_cast<double2*>(sm + lane * 8 + e) = make_double2(cf * al[e], cf * al[e + 1]);
+            sm[am_a8 + lane] = cf * al[8];
+        } else if (lane == 27) {
+            sm[243] = 0.0;                                   // the pad entry of the block
+        }
+        if (lane < 8) {
+            // rho / Jhat of corner (ca, cb, cc) (L147, Eq. 1)
+            const double wq = qV * ((wx[ca] * wy[cb]) * wz[cc]);
+            *reinterpret_cast<double2*>(sm + 244 + lane * 4) = make_double2(wq, wq * vh[0]);
+            *reinterpret_cast<double2*>(sm + 244 + lane * 4 + 2) = make_double2(wq * vh[1], wq * vh[2]);
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
         const size_t cell = ((size_t)i0 * g.ny + j0) * g.nz + k0;
-        // rho / Jhat per corner of the cell (L147, Eq. 1)
-        double* aj = a.AJ + cell * 32;
-#pragma unroll
-        for (int c = 0; c < 8; ++c) {
-            const double wq = qV * W[c];
-            atomicAdd(aj + c * 4 + 0, wq);
-            atomicAdd(aj + c * 4 + 1, wq * vh[0]);
-            atomicAdd(aj + c * 4 + 2, wq * vh[1]);
-            atomicAdd(aj + c * 4 + 3, wq * vh[2]);
+        if (lane == 0) {
+            bulk_reduce_add_f64(a.AM + cell * am_per_cell, sm, 244 * 8);
+            bulk_reduce_add_f64(a.AJ + cell * 32, sm + 244, 32 * 8);
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            // mover, Eq. (6)-(8) with periodic wrap
+            const double tx = vx + a.beta * Ep[0], ty = vy + a.beta * Ep[1], tz = vz + a.beta * Ep[2];
+            const double un = 2.0 * (al[0] * tx + al[1] * ty + al[2] * tz) - vx;
+            const double vn = 2.0 * (al[3] * tx + al[4] * ty + al[5] * tz) - vy;
+            const double wn = 2.0 * (al[6] * tx + al[7] * ty + al[8] * tz) - vz;
+            a.u[p] = un; a.v[p] = vn; a.w[p] = wn;
+            a.x[p] = wrap_periodic(x + a.dt * un, g.Lx);
+            a.y[p] = wrap_periodic(y + a.dt * vn, g.Ly);
+            a.z[p] = wrap_periodic(z + a.dt * wn, g.Lz);
+            my_leavers += 1;   // a stray stays outside the segment it is stored in
+            asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the staging block may be rewritten
         }
-        // the 27 weight-product classes of the cell (Eq. 3): class = kx*9 + ky*3 + kz, p?[0..2] = (w0^2, w0 w1, w1^2)
-        const double px[3] = {wx[0] * wx[0], wx[0] * wx[1], wx[1] * wx[1]};
-        const double py[3] = {wy[0] * wy[0], wy[0] * wy[1], wy[1] * wy[1]};
-        const double pz[3] = {wz[0] * wz[0], wz[0] * wz[1], wz[1] * wz[1]};
-        double* am = a.AM + cell * am_per_cell;
-#pragma unroll 1
-        for (int cls = 0; cls < 27; ++cls) {
-            const double cf = qbV * ((px[cls / 9] * py[(cls / 3) % 3]) * pz[cls % 3]);
-#pragma unroll
-            for (int e = 0; e < 8; ++e) atomicAdd(am + cls * 8 + e, cf * al[e]);
-            atomicAdd(am + am_a8 + cls, cf * al[8]);
-        }
-        // mover, Eq. (6)-(8) with periodic wrap
-        const double tx = vx + a.beta * Ep[0], ty = vy + a.beta * Ep[1], tz = vz + a.beta * Ep[2];
-        const double un = 2.0 * (al[0] * tx + al[1] * ty + al[2] * tz) - vx;
-        const double vn = 2.0 * (al[3] * tx + al[4] * ty + al[5] * tz) - vy;
-        const double wn = 2.0 * (al[6] * tx + al[7] * ty + al[8] * tz) - vz;
-        a.u[p] = un; a.v[p] = vn; a.w[p] = wn;
-        a.x[p] = wrap_periodic(x + a.dt * un, g.Lx);
-        a.y[p] = wrap_periodic(y + a.dt * vn, g.Ly);
-        a.z[p] = wrap_periodic(z + a.dt * wn, g.Lz);
-        my_leavers += 1;   // a stray stays outside the segment it is stored in
+        __syncwarp();
     }
-    if (a.leavers) {
-        my_leavers = __reduce_add_sync(0xffffffffu, my_leavers);
-        if (lane_id() == 0 && my_leavers) atomicAdd(a.leavers, (unsigned long long)my_leavers);
-    }
+    if (a.leavers && lane == 0 && my_leavers) atomicAdd(a.leavers, (unsigned long long)my_leavers);
 }

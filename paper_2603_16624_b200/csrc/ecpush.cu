@@ -85,7 +85,7 @@ struct ecsim_ctx {
     SpeciesHost* sp = nullptr;
     Workspace ws;
     int variant = ECSIM_VARIANT_FUSED;
-    double resort_fraction = 0.007;
+    double resort_fraction = 0.04;
     int timing = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     bool ev_valid = false;
@@ -573,7 +573,7 @@ static int push_and_moments_impl(ecsim_ctx* c, int n_list, const int* list, cons
         if (sp.state == ST_SEGMENTED && sp.leavers_pending) {
             CK(cudaEventSynchronize(sp.leavers_event));
             sp.leavers_pending = false;
-            // Rent or buy: a stray costs ~7.7 ns per step it stays a stray, a re-sort ~54 ps per particle (DESIGN.md
+            // Rent or buy: a stray costs ~1.4-2.2 ns per step it stays a stray, a re-sort ~54 ps per particle (DESIGN.md
             // §6.2).  Re-sort when the strays handled since the last sort plus those waiting now would have paid for it.
             if (sp.stray_debt + (double)c->h_leavers[s] > c->resort_fraction * (double)sp.n) sp.state = ST_UNSORTED;
             else sp.stray_debt += (double)c->h_leavers[s];
@@ -666,8 +666,8 @@ static int push_and_moments_impl(ecsim_ctx* c, int n_list, const int* list, cons
         CK(cudaEventRecord(c->ev_aux_done, c->aux));
         CK(cudaStreamWaitEvent(c->stream, c->ev_aux_done, 0));
     } else {
-        // strays first: they are deposited into the per-cell accumulators of their true cells (one 2.2 KB block
-        // per stray instead of eight node blocks), then one expansion serves everybody
+        // strays first: each is added to the per-cell accumulators of its true cell with one bulk reduction (a 2.2 KB
+        // block instead of atomics on eight node blocks), then one expansion serves everybody
         for (int i = 0; i < n_list; ++i) {
             const SpeciesHost& sp = c->sp[list[i]];
             if (sp.n == 0) continue;
@@ -676,7 +676,7 @@ static int push_and_moments_impl(ecsim_ctx* c, int n_list, const int* list, cons
             a.x = sp.x; a.y = sp.y; a.z = sp.z; a.u = sp.u; a.v = sp.v; a.w = sp.w; a.q = sp.q;
             a.E = E; a.B = B; a.beta = fa.sp[i].beta; a.dt = dt;
             a.AM = w.AM; a.AJ = fa.sp[i].AJ; a.leavers = fa.sp[i].leavers;
-            k_push_strays_to_cells<<<c->sm_count * 4, 128, 0, c->stream>>>(a, AM_PER_CELL, AM_A8);
+            k_push_strays_bulk<<<c->sm_count * 8, STRAY_WARPS * 32, 0, c->stream>>>(a, AM_PER_CELL, AM_A8);
             CK_LAUNCH();
             c->launches++;
         }
