@@ -254,5 +254,6 @@ k_push_strays_bulk(StrayArgs a, int am_per_cell, int am_a8)
         }
         __syncwarp();
     }
+    if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // every reduction of this warp has landed
     if (a.leavers && lane == 0 && my_leavers) atomicAdd(a.leavers, (unsigned long long)my_leavers);
 }
