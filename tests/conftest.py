@@ -24,3 +24,13 @@ def pytest_collection_modifyitems(config, items):
     for item in items:
         if "gpu" in item.keywords:
             item.add_marker(skip)
+
+
+@pytest.fixture(scope="session", autouse=True)
+def _native_libraries_are_built():
+    """libecpush.so (nvcc, sm_100a) and liboracle.so (gcc) are built in-tree if missing or stale.  Building the
+    product library is not a fallback: if nvcc fails the session fails."""
+    from paper_2603_16624_b200 import build as product_build
+    from oracle import build as oracle_build
+    product_build.build()
+    oracle_build.build()
