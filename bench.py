@@ -212,10 +212,14 @@ def run_product(args):
     rank, world, local = dist_env()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; libecpush has no CPU fallback")
+    if local == 0:
+        from paper_2603_16624_b200 import build as product_build
+        product_build.build()                     # in-tree, only if missing or stale; other ranks wait at the barrier below
     torch.cuda.set_device(local % torch.cuda.device_count())
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl")
+        dist.barrier()
     cfg = load_config(args)
     dev = torch.device("cuda")
     nsp = len(cfg.species)
