@@ -153,7 +153,7 @@ int ecsim_set_resort_fraction(ecsim_ctx *ctx, double fraction);
 int ecsim_set_fused_warps(ecsim_ctx *ctx, int warps);
 /* Number of x-plane slabs the FUSED step is cut into (1..16; 0 = default = 1).  With more than one slab the
  * expansion of slab s-1 (HBM bound; on a second stream owned by the context) runs beside the fused kernel of slab s
- * (FP64-issue bound; 12 warps x 144 registers so that an expansion CTA fits next to it on every SM); the caller's
+ * (FP64 bound; 12 warps x 144 registers so that an expansion CTA fits next to it on every SM); the caller's
  * stream waits for both before later work on it starts.  Results do not depend on the number.  On B200 one slab is
  * fastest; the knob stays for other grid shapes. */
 int ecsim_set_slabs(ecsim_ctx *ctx, int slabs);

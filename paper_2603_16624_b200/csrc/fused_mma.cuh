@@ -6,10 +6,9 @@
 //     34.1 / 37.1 / 32-33 TFLOP/s alone / alone / mixed), but one `mma.sync.m8n8k4.f64` carries 256
 //     FMAs in one instruction with two operand registers per lane, where 256 DFMA-FMAs as rank-1
 //     updates need ~100 operand doubles from shared memory.  Version 2 (DFMA) ran at 91 % of the
-//     shared-memory wavefront peak and 42 % of the FP64 pipe (profiles/r01a).  An FP64 instruction
-//     holds its scheduler's issue port for its pipe time (DMMA 16 cycles, DFMA 2; profiles/r01b), so
-//     every other instruction of this kernel costs FP64 throughput too: the code below is written
-//     for few instructions per particle.
+//     shared-memory wavefront peak and 42 % of the FP64 pipe (profiles/r01a).  Integer and shared-memory
+//     instructions issue underneath FP64 work, FFMA does not (profiles/r01e); what bounds this version is the
+//     latency of phase 1 at 3 warps per scheduler and the two phases contending for the one FP64 pipe.
 //   * One warp owns a contiguous range of cells, chosen from the segment tables so that every warp
 //     of the launch gets the same number of particles (+ a per-cell weight): a particle-balanced
 //     schedule that also serves non-uniform loads (Harris sheet).  A launch covers the cells
