@@ -636,7 +636,7 @@ static int push_and_moments_impl(ecsim_ctx* c, int n_list, const int* list, cons
     // With slabs (ecsim_set_slabs > 1) the fused kernels stay on the caller's stream as 12 warps x 144 registers,
     // and the expansions go to the context's second stream: one 128-thread expansion CTA fits beside a fused CTA
     // on every SM.  Measured on config 2 this overlap does not pay (1 slab 14.4 ms, 4 slabs 15.0, 8 slabs 15.3:
-    // the fused kernel is bound by instruction issue, so the expansion's instructions are not free, and it
+    // the fused kernel needs every warp slot and register of the SM, so the expansion beside it is not free, and it
     // loses its 168-register schedule); the default is one slab.  Other measured alternatives, all slower: fused
     // kernels on a high-priority stream with 8-24 SMs left free; persistent expansion CTAs.
     const int warps = c->fused_warps;
