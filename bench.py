@@ -54,7 +54,6 @@ def parse_args():
     ap.add_argument("--scale", default=None, help="nx,ny,nz override of the grid (tests / quick runs)")
     ap.add_argument("--variant", default="fused", choices=["fused", "atomic"])
     ap.add_argument("--fused-warps", type=int, default=0)
-    ap.add_argument("--slabs", type=int, default=0, help="x-plane slabs of the fused step (0 = library default)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -243,8 +242,6 @@ def run_product(args):
     ctx.set_variant(pk.VARIANT_FUSED if args.variant == "fused" else pk.VARIANT_ATOMIC)
     if args.fused_warps:
         ctx.set_fused_warps(args.fused_warps)
-    if args.slabs:
-        ctx.set_slabs(args.slabs)
     ctx.enable_timing(True)
     rho = torch.empty(nsp, cfg.nodes, dtype=torch.float64, device=dev)
     J = torch.empty(nsp, 3, cfg.nodes, dtype=torch.float64, device=dev)

@@ -47,7 +47,8 @@ enum ecsim_status {
     ECSIM_ERR_NOT_LOADED = -2,  /* species has no particles loaded */
     ECSIM_ERR_WORKSPACE = -3,   /* workspace missing or smaller than ecsim_workspace_bytes() */
     ECSIM_ERR_CUDA = -4,        /* a CUDA call failed; text via ecsim_last_error() */
-    ECSIM_ERR_NOMEM = -5        /* host allocation failed */
+    ECSIM_ERR_NOMEM = -5,       /* host allocation failed */
+    ECSIM_ERR_OVERFLOW = -6     /* resident species: a push found segments AND the overflow list full; particles were dropped */
 };
 
 /* `accumulate` argument of the push_and_moments calls. */
@@ -56,6 +57,13 @@ enum ecsim_accumulate {
     ECSIM_ACC_ALL = 1,   /* contributions are added to rho, Jhat and M (sum over species, L84) */
     ECSIM_ACC_M_ONLY = 2 /* added to M (mass matrices are summed over species, L59); rho and Jhat of this
                             species are overwritten (Jhat is kept per species, L129) */
+};
+
+/* Storage of the mass matrices (ecsim_set_m_layout). */
+enum ecsim_m_layout {
+    ECSIM_M_27 = 0, /* default: M[node][27][3][3], every neighbour slot (the north-star layout) */
+    ECSIM_M_14 = 1  /* the paper's symmetric storage (L73, L129): M14[node][14][3][3] = the slots o = 13..26 (self and the 13
+                       "upper" neighbours); slot o < 13 of node g is slot 26-o of node g + off(o) (M_NN' = M_N'N per component) */
 };
 
 /* Kernel variants of ecsim_push_and_moments (ecsim_set_variant). */
@@ -94,6 +102,9 @@ int ecsim_load_particles(ecsim_ctx *ctx, int species, int64_t n, double q_over_m
  * perm_out: device uint32[n], perm_out[new] = old index, or NULL. */
 int ecsim_sort_particles(ecsim_ctx *ctx, int species, int32_t *cell_count_out, uint32_t *perm_out);
 
+/* (A resident species -- ecsim_make_resident -- keeps itself sorted: ecsim_sort_particles and ecsim_cell_index
+ * return ECSIM_ERR_INVALID_ARG for it.) */
+
 /* Build the per-cell segment table (start[cells+1]) of a species whose arrays are ALREADY cell-sorted
  * (histogram + exclusive scan, no particle moves).  ecsim_push_and_moments does this by itself for a
  * species loaded with sorted != 0; calling it first keeps that set-up out of a timed step. */
@@ -123,6 +134,60 @@ int ecsim_push_and_moments(ecsim_ctx *ctx, int species, const double *E_theta, c
 int ecsim_push_and_moments_all(ecsim_ctx *ctx, const double *E_theta, const double *B, double dt, double theta,
                                double *rho, double *Jhat, double *M, int accumulate);
 
+/* The two halves of the step as separate calls (moment gathering -> field solve -> particle mover; in a
+ * real time loop E^{n+theta} comes out of the solve that the moments feed, L86).  Same kernels, same layouts, same
+ * conventions as ecsim_push_and_moments:
+ *   ecsim_moments  deposits rho, Jhat, M from the stored x, v (L49: "both evaluated at time n"); particles untouched;
+ *                  needs B^n only (alpha_p, Eq. 2).  Arguments as above.
+ *   ecsim_push     Eq. 6-8 with E^{n+theta} and the same B^n: v^{n+1}, x advanced and wrapped; no deposit.
+ * ecsim_moments followed by ecsim_push with the same B equals ecsim_push_and_moments (up to rounding order: none, the
+ * per-particle arithmetic is the same code).  The *_all forms take every species of the context in one pass. */
+int ecsim_moments(ecsim_ctx *ctx, int species, const double *B, double dt, double *rho, double *Jhat, double *M,
+                  int accumulate);
+int ecsim_moments_all(ecsim_ctx *ctx, const double *B, double dt, double *rho, double *Jhat, double *M, int accumulate);
+int ecsim_push(ecsim_ctx *ctx, int species, const double *E_theta, const double *B, double dt, double theta);
+int ecsim_push_all(ecsim_ctx *ctx, const double *E_theta, const double *B, double dt, double theta);
+
+/* RESIDENT species: the sort-preserving push (L149: the sort the paper could not realise).
+ * ecsim_make_resident bins a loaded species and copies it into two library-managed buffers inside dev_buf (device
+ * memory lent by the caller until ecsim_destroy / the next ecsim_load_particles of that species; 256-byte aligned,
+ * ecsim_resident_bytes(ctx, n, slack) large).  Each cell owns a segment of slots in both buffers: its particles plus
+ * max(8, slack * particles) spare slots.  From then on every push of that species (ecsim_push, ecsim_push_and_moments,
+ * *_all) reads one buffer and writes the other: particles that stay in their cell are written, compacted, to the front
+ * of the cell's segment, a particle that moves to another cell is written straight to the back of THAT cell's segment.
+ * Every step therefore starts from cell-sorted particles: no strays, no re-sort.  A particle whose new cell has no free
+ * slot goes to an overflow list (n/8 entries); the next call then lays the species out afresh (counted by
+ * ecsim_relayout_count).  The arrays given to ecsim_load_particles are not referenced after ecsim_make_resident returns
+ * and are NOT updated by pushes: read the species back with ecsim_export_particles (device arrays of n doubles each;
+ * cell-major order; also works, as a plain copy, for a species that is not resident).
+ * ecsim_make_resident synchronises the stream once (it checks the data-dependent slot count against the buffer);
+ * slack in [0, 4], typically 0.25.  All species of one *_all call must be of one kind (all resident or none). */
+size_t ecsim_resident_bytes(const ecsim_ctx *ctx, int64_t n_particles, double slack);
+int ecsim_make_resident(ecsim_ctx *ctx, int species, void *dev_buf, size_t bytes, double slack);
+int ecsim_export_particles(ecsim_ctx *ctx, int species, double *x, double *y, double *z, double *u, double *v,
+                           double *w, double *q);
+int64_t ecsim_relayout_count(const ecsim_ctx *ctx);
+
+/* Diagnostic moments of one species, the quantities ECsim writes with its I/O (L121 "plasma density, current, pressure,
+ * and heat flux"; L147 computeCharge / computeCurrent: "The diagnostic charge current differs from J-hat, as it excludes
+ * the effect of velocity rotation").  With the same weights W_pN as Eq. (1) (the paper prints no formulas; readings
+ * R22-R24 of DESIGN.md):
+ *   rho [nodes]     = sum_p q_p W_pN / V_N
+ *   J   [3][nodes]  = sum_p q_p W_pN v_p / V_N                      (no alpha_p)
+ *   P   [6][nodes]  = sum_p q_p W_pN v_p^i v_p^j / V_N              components xx, xy, xz, yy, yz, zz
+ *   Q   [3][nodes]  = sum_p q_p W_pN (|v_p|^2 / 2) v_p^i / V_N
+ * Device outputs, overwritten; any may be NULL.  Particles untouched.  Works for dense and resident species. */
+int ecsim_diagnostics(ecsim_ctx *ctx, int species, double *rho, double *J, double *P, double *Q);
+
+/* Mass-matrix storage for all later deposit calls and for ecsim_apply_M: enum ecsim_m_layout.  With ECSIM_M_14 the M
+ * argument of the deposit calls is M14[nodes][14][3][3] (half the bytes; VARIANT_ATOMIC supports ECSIM_M_27 only). */
+int ecsim_set_m_layout(ecsim_ctx *ctx, int layout);
+
+/* out_N = sum_N' M_NN' E_N' over the 27 neighbours of every node (Eq. 4-5: the mass-matrix term of the
+ * field equations, applied once per Krylov iteration of the implicit solve).  M in the context's current layout;
+ * E, out: device [3][nodes], E != out; accumulate != 0: out += . */
+int ecsim_apply_M(ecsim_ctx *ctx, const double *M, const double *E, double *out, int accumulate);
+
 /* Same step with HOST buffers: copies particles and fields to device staging (carved from the
  * workspace, which must be ecsim_host_step_workspace_bytes() large), runs the step, copies particles
  * and moments back, and synchronises the stream.  Host arrays: x..w in/out [n], q in [n], E/B in,
@@ -148,16 +213,9 @@ int ecsim_set_variant(ecsim_ctx *ctx, int variant);
 
 /* Tuning knobs: fraction of a species that may sit outside its cell segment before the next step re-sorts
  * (default 0.04); warps per CTA of the fused kernel (8, 12 or 16, with 224, 168 or 128 registers per thread;
- * default 12; always 12 x 144 when slabs overlap). */
+ * default 12). */
 int ecsim_set_resort_fraction(ecsim_ctx *ctx, double fraction);
 int ecsim_set_fused_warps(ecsim_ctx *ctx, int warps);
-/* Number of x-plane slabs the FUSED step is cut into (1..16; 0 = default = 1).  With more than one slab the
- * expansion of slab s-1 (HBM bound; on a second stream owned by the context) runs beside the fused kernel of slab s
- * (FP64 bound; 12 warps x 144 registers so that an expansion CTA fits next to it on every SM); the caller's
- * stream waits for both before later work on it starts.  Results do not depend on the number.  On B200 one slab is
- * fastest; the knob stays for other grid shapes. */
-int ecsim_set_slabs(ecsim_ctx *ctx, int slabs);
-
 /* Instrumentation.  ecsim_enable_timing(1) records CUDA events around the deposit/push kernel of every
  * ecsim_push_and_moments call; ecsim_kernel_ms() SYNCHRONISES on the last pair and returns its time.
  * ecsim_launch_count() = kernels + memsets this context has enqueued so far;
@@ -166,6 +224,7 @@ int ecsim_enable_timing(ecsim_ctx *ctx, int on);
 int ecsim_kernel_ms(ecsim_ctx *ctx, float *ms_out);
 int64_t ecsim_launch_count(const ecsim_ctx *ctx);
 int64_t ecsim_stray_count(ecsim_ctx *ctx);
+int64_t ecsim_leaver_count(ecsim_ctx *ctx);       /* particles whose cell changed in the last push (synchronises the stream) */
 int64_t ecsim_resort_count(const ecsim_ctx *ctx); /* re-sorts ecsim_push_and_moments triggered so far */
 
 /* FP64 FMA throughput of the device (dependent-chain DFMA kernel, `iters` x 128 FMAs per thread), the

@@ -1,6 +1,6 @@
 """CPU oracle of the ECsim particle hot path -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
 
-`oracle.step` / `oracle.cells` / `oracle.apply_M` wrap the plain C restatement of the paper's
+`oracle.step` / `oracle.cells` / `oracle.apply_M` / `oracle.diagnostics` wrap the plain C restatement of the paper's
 equations in `ecsim_oracle.c`; `oracle.dense` is the hat-function definition written out in
 numpy for tiny grids.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
 `--impl reference` legs may import this package; it imports nothing from the CUDA package.
@@ -33,6 +33,9 @@ def lib():
             [ctypes.c_int] * 3 + [ctypes.c_double] * 3 + [ctypes.c_int64] + [_D] * 3 + [_I32, _I32])
         _lib.ecsim_oracle_apply_M.restype = ctypes.c_int
         _lib.ecsim_oracle_apply_M.argtypes = [ctypes.c_int] * 3 + [_D] * 3
+        _lib.ecsim_oracle_diagnostics.restype = ctypes.c_int
+        _lib.ecsim_oracle_diagnostics.argtypes = ([ctypes.c_int] * 3 + [ctypes.c_double] * 3 + [ctypes.c_int64]
+                                                  + [_D] * 7 + [_D] * 4 + [_D] * 4)
     return _lib
 
 
@@ -91,3 +94,28 @@ def apply_M(grid, M: np.ndarray, E: np.ndarray) -> np.ndarray:
     rc = lib().ecsim_oracle_apply_M(nx, ny, nz, _p(M), _p(E), _p(out))
     assert rc == 0
     return out
+
+
+class Diagnostics:
+    """rho [nodes], J [3][nodes] (un-rotated), P [6][nodes] (xx,xy,xz,yy,yz,zz), Q [3][nodes] and |addend| sums."""
+
+    def __init__(self, nodes: int, with_abs: bool = True):
+        self.rho = np.zeros(nodes)
+        self.J = np.zeros((3, nodes))
+        self.P = np.zeros((6, nodes))
+        self.Q = np.zeros((3, nodes))
+        self.rho_abs = np.zeros(nodes) if with_abs else None
+        self.J_abs = np.zeros((3, nodes)) if with_abs else None
+        self.P_abs = np.zeros((6, nodes)) if with_abs else None
+        self.Q_abs = np.zeros((3, nodes)) if with_abs else None
+
+
+def diagnostics(grid, part: dict, diag: Diagnostics):
+    """Diagnostic moments of one species (R22-R24), accumulated into `diag`."""
+    nx, ny, nz, dx, dy, dz = grid
+    n = part["x"].shape[0]
+    rc = lib().ecsim_oracle_diagnostics(
+        nx, ny, nz, dx, dy, dz, n, _p(part["x"]), _p(part["y"]), _p(part["z"]), _p(part["u"]), _p(part["v"]),
+        _p(part["w"]), _p(part["q"]), _p(diag.rho), _p(diag.J), _p(diag.P), _p(diag.Q),
+        _p(diag.rho_abs), _p(diag.J_abs), _p(diag.P_abs), _p(diag.Q_abs))
+    assert rc == 0

@@ -229,3 +229,61 @@ int ecsim_oracle_apply_M(int nx, int ny, int nz, const double *M, const double *
             }
     return 0;
 }
+
+/*
+ * Diagnostic moments for I/O ("plasma density, current, pressure, and heat flux ... interpolating
+ * particle to the grid"; L147 computeCharge / computeCurrent: "charge density, charge current, and pressure tensor.
+ * The diagnostic charge current differs from J-hat, as it excludes the effect of velocity rotation").  The paper
+ * prints no formula for them; the readings are DESIGN.md R22-R24: with the same 2x2x2 weights W_pN as Eq. (1),
+ *     rho_N  = (1/V_N) sum_p q_p W_pN                               (the same rho as ecsim_oracle_step)
+ *     J_N    = (1/V_N) sum_p q_p W_pN v_p                           (no alpha_p: un-rotated)
+ *     P_N^ij = (1/V_N) sum_p q_p W_pN v_p^i v_p^j                   6 components xx, xy, xz, yy, yz, zz
+ *     Q_N^i  = (1/V_N) sum_p q_p W_pN (|v_p|^2 / 2) v_p^i           heat (energy) flux
+ * Per particle, in input order; outputs accumulated into (+=), caller zeroes; *_abs optional |addend| sums.
+ * Layout: rho[n]; J[c*nodes + n]; P[c*nodes + n], c = 0..5; Q[c*nodes + n].
+ */
+int ecsim_oracle_diagnostics(int nx, int ny, int nz, double dx, double dy, double dz, int64_t n,
+                             const double *x, const double *y, const double *z,
+                             const double *u, const double *v, const double *w, const double *q,
+                             double *rho, double *J, double *P, double *Q,
+                             double *rho_abs, double *J_abs, double *P_abs, double *Q_abs)
+{
+    const int64_t nodes = (int64_t)nx * ny * nz;
+    const double rdx = 1.0 / dx, rdy = 1.0 / dy, rdz = 1.0 / dz;
+    const double invV = 1.0 / (dx * dy * dz);
+    for (int64_t p = 0; p < n; ++p) {
+        const double sx = x[p] * rdx, sy = y[p] * rdy, sz = z[p] * rdz;
+        const int i0 = lower_node(sx, nx), j0 = lower_node(sy, ny), k0 = lower_node(sz, nz);
+        const int in[2] = {i0, (i0 + 1) % nx};
+        const int jn[2] = {j0, (j0 + 1) % ny};
+        const int kn[2] = {k0, (k0 + 1) % nz};
+        const double xi = sx - i0, eta = sy - j0, zeta = sz - k0;
+        const double wx[2] = {1.0 - xi, xi}, wy[2] = {1.0 - eta, eta}, wz[2] = {1.0 - zeta, zeta};
+        const double vv[3] = {u[p], v[p], w[p]};
+        const double pp[6] = {vv[0] * vv[0], vv[0] * vv[1], vv[0] * vv[2], vv[1] * vv[1], vv[1] * vv[2], vv[2] * vv[2]};
+        const double half_v2 = 0.5 * ((vv[0] * vv[0] + vv[1] * vv[1]) + vv[2] * vv[2]);
+        const double qV = q[p] * invV;
+        for (int a = 0; a < 2; ++a)
+            for (int b = 0; b < 2; ++b)
+                for (int c = 0; c < 2; ++c) {
+                    const int64_t g = ((int64_t)in[a] * ny + jn[b]) * nz + kn[c];
+                    const double dr = qV * ((wx[a] * wy[b]) * wz[c]);
+                    rho[g] += dr;
+                    if (rho_abs) rho_abs[g] += fabs(dr);
+                    for (int r = 0; r < 3; ++r) {
+                        const double dj = dr * vv[r];
+                        J[r * nodes + g] += dj;
+                        if (J_abs) J_abs[r * nodes + g] += fabs(dj);
+                        const double dq = dr * (half_v2 * vv[r]);
+                        Q[r * nodes + g] += dq;
+                        if (Q_abs) Q_abs[r * nodes + g] += fabs(dq);
+                    }
+                    for (int r = 0; r < 6; ++r) {
+                        const double dp = dr * pp[r];
+                        P[r * nodes + g] += dp;
+                        if (P_abs) P_abs[r * nodes + g] += fabs(dp);
+                    }
+                }
+    }
+    return 0;
+}

@@ -18,4 +18,6 @@ from .binding import (  # noqa: F401
     ACC_NONE,
     ACC_ALL,
     ACC_M_ONLY,
+    M_27,
+    M_14,
 )

@@ -20,6 +20,8 @@ VARIANT_FUSED = 1
 ACC_NONE = 0
 ACC_ALL = 1
 ACC_M_ONLY = 2
+M_27 = 0
+M_14 = 1
 
 _c = ctypes
 _P = _c.c_void_p
@@ -38,7 +40,7 @@ def declared_symbols() -> list:
     """Names of every function include/ecpush.h declares (used by the ABI test)."""
     text = open(HEADER).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(ecsim_[a-z0-9_]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(ecsim_[A-Za-z0-9_]+)\s*\(", text)))
 
 
 _PROTOS = {
@@ -52,6 +54,16 @@ _PROTOS = {
     "ecsim_cell_index": (_c.c_int, [_P, _c.c_int, _P]),
     "ecsim_push_and_moments": (_c.c_int, [_P, _c.c_int, _P, _P, _c.c_double, _c.c_double, _P, _P, _P, _c.c_int]),
     "ecsim_push_and_moments_all": (_c.c_int, [_P, _P, _P, _c.c_double, _c.c_double, _P, _P, _P, _c.c_int]),
+    "ecsim_moments": (_c.c_int, [_P, _c.c_int, _P, _c.c_double, _P, _P, _P, _c.c_int]),
+    "ecsim_moments_all": (_c.c_int, [_P, _P, _c.c_double, _P, _P, _P, _c.c_int]),
+    "ecsim_push": (_c.c_int, [_P, _c.c_int, _P, _P, _c.c_double, _c.c_double]),
+    "ecsim_push_all": (_c.c_int, [_P, _P, _P, _c.c_double, _c.c_double]),
+    "ecsim_resident_bytes": (_c.c_size_t, [_P, _c.c_int64, _c.c_double]),
+    "ecsim_make_resident": (_c.c_int, [_P, _c.c_int, _P, _c.c_size_t, _c.c_double]),
+    "ecsim_export_particles": (_c.c_int, [_P, _c.c_int] + [_P] * 7),
+    "ecsim_relayout_count": (_c.c_int64, [_P]),
+    "ecsim_apply_M": (_c.c_int, [_P, _P, _P, _P, _c.c_int]),
+    "ecsim_diagnostics": (_c.c_int, [_P, _c.c_int, _P, _P, _P, _P]),
     "ecsim_host_step_workspace_bytes": (_c.c_size_t, [_P, _c.c_int64]),
     "ecsim_push_and_moments_host": (_c.c_int, [_P, _c.c_int64, _c.c_double, _c.c_int] + [_P] * 9 +
                                     [_c.c_double, _c.c_double, _P, _P, _P, _c.c_int]),
@@ -61,11 +73,12 @@ _PROTOS = {
     "ecsim_set_variant": (_c.c_int, [_P, _c.c_int]),
     "ecsim_set_resort_fraction": (_c.c_int, [_P, _c.c_double]),
     "ecsim_set_fused_warps": (_c.c_int, [_P, _c.c_int]),
-    "ecsim_set_slabs": (_c.c_int, [_P, _c.c_int]),
+    "ecsim_set_m_layout": (_c.c_int, [_P, _c.c_int]),
     "ecsim_enable_timing": (_c.c_int, [_P, _c.c_int]),
     "ecsim_kernel_ms": (_c.c_int, [_P, _c.POINTER(_c.c_float)]),
     "ecsim_launch_count": (_c.c_int64, [_P]),
     "ecsim_stray_count": (_c.c_int64, [_P]),
+    "ecsim_leaver_count": (_c.c_int64, [_P]),
     "ecsim_resort_count": (_c.c_int64, [_P]),
     "ecsim_probe_fp64": (_c.c_int, [_P, _c.c_int, _c.POINTER(_c.c_double), _c.POINTER(_c.c_float)]),
     "ecsim_destroy": (_c.c_int, [_P]),
@@ -138,6 +151,7 @@ class Ecsim:
         self.h = h
         self._ws = None
         self._keep = {}
+        self._resident = {}
 
     # -- workspace -----------------------------------------------------------------------------
     def workspace_bytes(self, n_max: int) -> int:
@@ -161,6 +175,7 @@ class Ecsim:
         n = int(part["x"].numel())
         ptrs = [_dptr(part[k], f64) for k in ("x", "y", "z", "u", "v", "w", "q")]
         self._keep[species] = part
+        self._resident.pop(species, None)
         _check(self.L.ecsim_load_particles(self.h, species, n, qom, *ptrs, 1 if sorted else 0),
                "ecsim_load_particles")
 
@@ -186,6 +201,62 @@ class Ecsim:
         _check(self.L.ecsim_push_and_moments_all(self.h, _dptr(E, f64), _dptr(B, f64), dt, theta,
                                                  _dptr(rho, f64), _dptr(Jhat, f64), _dptr(M, f64),
                                                  int(accumulate)), "ecsim_push_and_moments_all")
+
+    # -- the two halves as separate calls (moment gathering -> field solve -> mover) -----------
+    def moments(self, species: int, B, dt: float, rho, Jhat, M, accumulate: int = 0):
+        f64 = self.torch.float64
+        _check(self.L.ecsim_moments(self.h, species, _dptr(B, f64), dt, _dptr(rho, f64), _dptr(Jhat, f64),
+                                    _dptr(M, f64), int(accumulate)), "ecsim_moments")
+
+    def moments_all(self, B, dt: float, rho, Jhat, M, accumulate: int = 0):
+        f64 = self.torch.float64
+        _check(self.L.ecsim_moments_all(self.h, _dptr(B, f64), dt, _dptr(rho, f64), _dptr(Jhat, f64),
+                                        _dptr(M, f64), int(accumulate)), "ecsim_moments_all")
+
+    def push(self, species: int, E, B, dt: float, theta: float):
+        f64 = self.torch.float64
+        _check(self.L.ecsim_push(self.h, species, _dptr(E, f64), _dptr(B, f64), dt, theta), "ecsim_push")
+
+    def push_all(self, E, B, dt: float, theta: float):
+        f64 = self.torch.float64
+        _check(self.L.ecsim_push_all(self.h, _dptr(E, f64), _dptr(B, f64), dt, theta), "ecsim_push_all")
+
+    # -- resident species: the sort-preserving push ---------------------------------------------------------
+    def resident_bytes(self, n: int, slack: float = 0.25) -> int:
+        return int(self.L.ecsim_resident_bytes(self.h, n, slack))
+
+    def make_resident(self, species: int, slack: float = 0.25):
+        """Let torch allocate the species' gapped double buffers and hand the species over to the library."""
+        part = self._keep[species]
+        nbytes = self.resident_bytes(int(part["x"].numel()), slack)
+        buf = self.torch.empty(nbytes + 256, dtype=self.torch.uint8, device="cuda")
+        off = (-buf.data_ptr()) % 256
+        _check(self.L.ecsim_make_resident(self.h, species, _P(buf.data_ptr() + off), nbytes, slack),
+               "ecsim_make_resident")
+        self._resident[species] = buf
+        return nbytes
+
+    def export_particles(self, species: int, out: dict):
+        f64 = self.torch.float64
+        ptrs = [_dptr(out[k], f64) for k in ("x", "y", "z", "u", "v", "w", "q")]
+        _check(self.L.ecsim_export_particles(self.h, species, *ptrs), "ecsim_export_particles")
+
+    def relayout_count(self) -> int:
+        return int(self.L.ecsim_relayout_count(self.h))
+
+    def diagnostics(self, species: int, rho, J, P, Q):
+        f64 = self.torch.float64
+        _check(self.L.ecsim_diagnostics(self.h, species, _dptr(rho, f64), _dptr(J, f64), _dptr(P, f64), _dptr(Q, f64)),
+               "ecsim_diagnostics")
+
+    # -- mass-matrix storage and operator ---------------------------------------------------------------------
+    def set_m_layout(self, layout: int):
+        _check(self.L.ecsim_set_m_layout(self.h, layout), "ecsim_set_m_layout")
+
+    def apply_M(self, M, E, out, accumulate: bool = False):
+        f64 = self.torch.float64
+        _check(self.L.ecsim_apply_M(self.h, _dptr(M, f64), _dptr(E, f64), _dptr(out, f64), 1 if accumulate else 0),
+               "ecsim_apply_M")
 
     def push_and_moments_host(self, qom: float, sorted: bool, part: dict, E, B, dt: float, theta: float,
                               rho, Jhat, M, accumulate: int = 0):
@@ -230,9 +301,6 @@ class Ecsim:
     def set_fused_warps(self, w: int):
         _check(self.L.ecsim_set_fused_warps(self.h, w), "ecsim_set_fused_warps")
 
-    def set_slabs(self, n: int):
-        _check(self.L.ecsim_set_slabs(self.h, n), "ecsim_set_slabs")
-
     def enable_timing(self, on: bool = True):
         _check(self.L.ecsim_enable_timing(self.h, 1 if on else 0), "ecsim_enable_timing")
 
@@ -246,6 +314,9 @@ class Ecsim:
 
     def stray_count(self) -> int:
         return int(self.L.ecsim_stray_count(self.h))
+
+    def leaver_count(self) -> int:
+        return int(self.L.ecsim_leaver_count(self.h))
 
     def resort_count(self) -> int:
         return int(self.L.ecsim_resort_count(self.h))
@@ -261,6 +332,7 @@ class Ecsim:
             self.h = None
             self._ws = None
             self._keep = {}
+            self._resident = {}
 
     def __del__(self):
         try:

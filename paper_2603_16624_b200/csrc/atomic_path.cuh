@@ -17,8 +17,9 @@ struct AtomicArgs {
     const double *E, *B;        // [3][nodes]
     double beta;                // q dt / (2 m) (L55)
     double dt;
-    double *rho, *J, *M;        // any may be null
+    double *rho, *J, *M;        // any may be null (deposit skipped)
     unsigned long long* leavers; // optional: particles whose cell changed in the push
+    int do_push;                // 0: deposit only, x and v untouched (ecsim_moments)
 };
 
 template <bool USE_LIST>
@@ -107,6 +108,7 @@ k_push_moments_atomic(AtomicArgs a)
             }
         }
 
+        if (!a.do_push) continue;
         // mover, Eq. (6)-(8) with periodic wrap
         const double tx = vx + a.beta * Ep[0], ty = vy + a.beta * Ep[1], tz = vz + a.beta * Ep[2];
         const double vbx = al[0] * tx + al[1] * ty + al[2] * tz;
@@ -149,6 +151,7 @@ struct StrayArgs {
     double* AM;                 // [cells][AM_PER_CELL]
     double* AJ;                 // [cells][8][4] of this species
     unsigned long long* leavers;
+    int do_deposit, do_push;    // ecsim_moments: (1, 0); ecsim_push: (0, 1); ecsim_push_and_moments: (1, 1)
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -219,7 +222,9 @@ k_push_strays_bulk(StrayArgs a, int am_per_cell, int am_a8)
         const double fy = (ky == 0 ? wy[0] * wy[0] : ky == 1 ? wy[0] * wy[1] : wy[1] * wy[1]);
         const double fz = (kz == 0 ? wz[0] * wz[0] : kz == 1 ? wz[0] * wz[1] : wz[1] * wz[1]);
         const double cf = qbV * ((fx * fy) * fz);
-        if (lane < 27) {
+        if (!a.do_deposit) {
+            // push only
+        } else if (lane < 27) {
 #pragma unroll
             for (int e = 0; e < 8; e += 2)
                 *reinterpret_cast<double2*>(sm + lane * 8 + e) = make_double2(cf * al[e], cf * al[e + 1]);
@@ -227,7 +232,7 @@ k_push_strays_bulk(StrayArgs a, int am_per_cell, int am_a8)
         } else if (lane == 27) {
             sm[243] = 0.0;                                   // the pad entry of the block
         }
-        if (lane < 8) {
+        if (a.do_deposit && lane < 8) {
             // rho / Jhat of corner (ca, cb, cc) (L147, Eq. 1)
             const double wq = qV * ((wx[ca] * wy[cb]) * wz[cc]);
             *reinterpret_cast<double2*>(sm + 244 + lane * 4) = make_double2(wq, wq * vh[0]);
@@ -237,9 +242,13 @@ k_push_strays_bulk(StrayArgs a, int am_per_cell, int am_a8)
         __syncwarp();
         const size_t cell = ((size_t)i0 * g.ny + j0) * g.nz + k0;
         if (lane == 0) {
-            bulk_reduce_add_f64(a.AM + cell * am_per_cell, sm, 244 * 8);
-            bulk_reduce_add_f64(a.AJ + cell * 32, sm + 244, 32 * 8);
+            if (a.do_deposit) {
+                bulk_reduce_add_f64(a.AM + cell * am_per_cell, sm, 244 * 8);
+                bulk_reduce_add_f64(a.AJ + cell * 32, sm + 244, 32 * 8);
+            }
             asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        }
+        if (lane == 0 && a.do_push) {
             // mover, Eq. (6)-(8) with periodic wrap
             const double tx = vx + a.beta * Ep[0], ty = vy + a.beta * Ep[1], tz = vz + a.beta * Ep[2];
             const double un = 2.0 * (al[0] * tx + al[1] * ty + al[2] * tz) - vx;
@@ -250,10 +259,50 @@ k_push_strays_bulk(StrayArgs a, int am_per_cell, int am_a8)
             a.y[p] = wrap_periodic(y + a.dt * vn, g.Ly);
             a.z[p] = wrap_periodic(z + a.dt * wn, g.Lz);
             my_leavers += 1;   // a stray stays outside the segment it is stored in
-            asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the staging block may be rewritten
         }
+        if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the staging block may be rewritten
         __syncwarp();
     }
     if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // every reduction of this warp has landed
     if (a.leavers && lane == 0 && my_leavers) atomicAdd(a.leavers, (unsigned long long)my_leavers);
+}
+
+// Strays of the diagnostics pass (dense layout): one thread per listed particle, 8 corners x 13 atomics onto the node
+// arrays, after the expansion wrote them.
+struct DiagStrayArgs {
+    Geom g;
+    const uint32_t* list;
+    const uint32_t* list_count;
+    const double *x, *y, *z, *u, *v, *w, *q;
+    double *rho, *J, *P, *Q;
+};
+
+__global__ void __launch_bounds__(128)
+k_diag_strays(DiagStrayArgs a)
+{
+    const Geom& g = a.g;
+    const size_t count = (size_t)*a.list_count;
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < count; t += stride) {
+        const size_t p = a.list[t];
+        const double sx = a.x[p] * g.rdx, sy = a.y[p] * g.rdy, sz = a.z[p] * g.rdz;
+        const int i0 = lower_node(sx, g.nx), j0 = lower_node(sy, g.ny), k0 = lower_node(sz, g.nz);
+        const int i1 = (i0 + 1 == g.nx) ? 0 : i0 + 1, j1 = (j0 + 1 == g.ny) ? 0 : j0 + 1, k1 = (k0 + 1 == g.nz) ? 0 : k0 + 1;
+        const double xi = sx - i0, eta = sy - j0, zeta = sz - k0;
+        const double wx[2] = {1.0 - xi, xi}, wy[2] = {1.0 - eta, eta}, wz[2] = {1.0 - zeta, zeta};
+        const double vx = a.u[p], vy = a.v[p], vz = a.w[p];
+        const double h = 0.5 * ((vx * vx + vy * vy) + vz * vz);
+        const double col[13] = {1.0, vx, vy, vz, vx * vx, vx * vy, vx * vz, vy * vy, vy * vz, vz * vz, h * vx, h * vy, h * vz};
+        const double qV = a.q[p] * g.invV;
+#pragma unroll 1
+        for (int c = 0; c < 8; ++c) {
+            const int ia = (c >> 2) & 1, ib = (c >> 1) & 1, ic = c & 1;
+            const long long n = ((long long)(ia ? i1 : i0) * g.ny + (ib ? j1 : j0)) * g.nz + (ic ? k1 : k0);
+            const double dr = qV * ((wx[ia] * wy[ib]) * wz[ic]);
+            if (a.rho) atomicAdd(a.rho + n, dr);
+            if (a.J) for (int r = 0; r < 3; ++r) atomicAdd(a.J + (size_t)r * g.nodes + n, dr * col[1 + r]);
+            if (a.P) for (int r = 0; r < 6; ++r) atomicAdd(a.P + (size_t)r * g.nodes + n, dr * col[4 + r]);
+            if (a.Q) for (int r = 0; r < 3; ++r) atomicAdd(a.Q + (size_t)r * g.nodes + n, dr * col[10 + r]);
+        }
+    }
 }

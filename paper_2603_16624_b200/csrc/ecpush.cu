@@ -1,6 +1,6 @@
-// ecpush.cu -- C ABI of libecpush (include/ecpush.h): context, workspace, orchestration of the
-// sm_100a kernels in sort.cuh / fused.cuh / atomic_path.cuh.  Product code: no CPU fallback, no
-// code shared with oracle/.  Every entry point returns an ecsim_status and never throws.
+// ecpush.cu -- C ABI of libecpush (include/ecpush.h): context, workspace, orchestration of the sm_100a kernels in
+// sort.cuh / fused_mma.cuh / resident.cuh / atomic_path.cuh / expand*.cuh / apply_m.cuh.  Product code: no CPU
+// fallback, no code shared with oracle/.  Every entry point returns an ecsim_status and never throws.
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdio.h>
@@ -15,6 +15,8 @@
 #include "fused_mma.cuh"
 #include "expand.cuh"
 #include "expand_tma.cuh"
+#include "resident.cuh"
+#include "apply_m.cuh"
 #include "probe.cuh"
 
 // --------------------------------------------------------------------------------------------
@@ -33,10 +35,23 @@ static int cuda_fail(cudaError_t e, const char* what, int line)
     } while (0)
 #define CK_LAUNCH() CK(cudaGetLastError())
 
-#define ECSIM_MAX_SLABS 16
-#define ECPUSH_OVERLAP_REGS 144   // 12 warps x 144 leave 10240 registers: one 128-thread x 64-register k_expand_M_stream CTA
-
 enum SortState { ST_UNSORTED = 0, ST_DECLARED = 1, ST_SEGMENTED = 2 };
+
+// A RESIDENT species (ecsim_make_resident): library-managed gapped double buffers in memory the caller lent
+// (resident.cuh; LAYOUT_GAPPED of fused_mma.cuh).
+struct Resident {
+    bool on = false;
+    uint32_t cap_bound = 0;         // slots per array the lent buffer can hold
+    double slack = 0.25;
+    double* buf[2][7] = {};         // two buffers of x,y,z,u,v,w,q
+    uint32_t* seg = nullptr;        // [cells+1] first slot of every cell's segment (both buffers)
+    uint32_t* F[2] = {};            // [cells] front runs
+    uint32_t* R[2] = {};            // [cells] back runs (arrivals of the last push)
+    int cur = 0;                    // buffer that holds the species now
+    double* ovf = nullptr;          // [7][ovf_cap] overflow list of the last push
+    uint32_t ovf_cap = 0;
+    uint32_t* ovf_count = nullptr;  // device counter
+};
 
 struct SpeciesHost {
     bool loaded = false;
@@ -46,8 +61,9 @@ struct SpeciesHost {
     int state = ST_UNSORTED;
     double stray_debt = 0.0;        // strays processed since the last sort, summed over the steps
     bool nearly_sorted = false;     // the arrays were cell-sorted before the last pushes (a re-sort, not a first sort)
-    bool leavers_pending = false;   // an async copy of the leaver counter is in flight
+    bool leavers_pending = false;   // an async copy of the leaver / overflow counters is in flight
     cudaEvent_t leavers_event = nullptr;
+    Resident res;
 };
 
 struct Workspace {
@@ -66,7 +82,7 @@ struct Workspace {
     uint32_t* tile_scan = nullptr;   // its exclusive scan (+1)
     uint32_t* tile_sums = nullptr;   // block sums of that scan
     uint32_t* stray_list = nullptr;  // [n_species][n_max]
-    double* AM = nullptr;            // [cells][243]
+    double* AM = nullptr;            // [cells][AM_PER_CELL = 244]
     double* AJ = nullptr;            // [n_species][cells][32]
     uint32_t* stray_count = nullptr; // [n_species]
     unsigned long long* leavers = nullptr; // [n_species]
@@ -78,10 +94,6 @@ struct ecsim_ctx {
     Geom g;
     int n_species = 0;
     cudaStream_t stream = nullptr;
-    cudaStream_t aux = nullptr;               // expansion of slab s-1 runs here while slab s is in the fused kernel
-    cudaEvent_t ev_slab[ECSIM_MAX_SLABS] = {};
-    cudaEvent_t ev_aux_done = nullptr;
-    int slabs = 0;                            // 0 = automatic
     SpeciesHost* sp = nullptr;
     Workspace ws;
     int variant = ECSIM_VARIANT_FUSED;
@@ -94,9 +106,12 @@ struct ecsim_ctx {
     int fused_warps = 12;
     unsigned long long* h_leavers = nullptr;  // pinned [n_species]
     uint32_t* h_strays = nullptr;             // pinned [n_species]
+    uint32_t* h_ovf = nullptr;                // pinned [n_species]: overflow count of the last resident push
     int last_call_species[ECSIM_MAX_SPECIES];
     int last_call_n = 0;
     int64_t resorts = 0;
+    int64_t relayouts = 0;
+    int m_layout = ECSIM_M_27;
 };
 
 static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
@@ -164,6 +179,7 @@ extern "C" const char* ecsim_strerror(int status)
     case ECSIM_ERR_WORKSPACE: return "workspace missing or too small";
     case ECSIM_ERR_CUDA: return "CUDA call failed (see ecsim_last_error)";
     case ECSIM_ERR_NOMEM: return "host allocation failed";
+    case ECSIM_ERR_OVERFLOW: return "resident species: segments and overflow list full, particles were dropped";
     default: return "unknown status";
     }
 }
@@ -198,20 +214,17 @@ extern "C" int ecsim_init_grid(ecsim_ctx** ctx, int nx, int ny, int nz, double d
     c->sm_count = prop.multiProcessorCount;
     cudaError_t e = cudaEventCreate(&c->ev0);
     if (e == cudaSuccess) e = cudaEventCreate(&c->ev1);
-    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->aux, cudaStreamNonBlocking);
-    for (int k = 0; k < ECSIM_MAX_SLABS && e == cudaSuccess; ++k)
-        e = cudaEventCreateWithFlags(&c->ev_slab[k], cudaEventDisableTiming);
-    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_aux_done, cudaEventDisableTiming);
     for (int s = 0; s < n_species && e == cudaSuccess; ++s)
         e = cudaEventCreateWithFlags(&c->sp[s].leavers_event, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaMallocHost(&c->h_leavers, sizeof(unsigned long long) * n_species);
     if (e == cudaSuccess) e = cudaMallocHost(&c->h_strays, sizeof(uint32_t) * n_species);
+    if (e == cudaSuccess) e = cudaMallocHost(&c->h_ovf, sizeof(uint32_t) * n_species);
     if (e != cudaSuccess) {
         int rc = cuda_fail(e, "context set-up", __LINE__);
         ecsim_destroy(c);
         return rc;
     }
-    for (int s = 0; s < n_species; ++s) { c->h_leavers[s] = 0; c->h_strays[s] = 0; }
+    for (int s = 0; s < n_species; ++s) { c->h_leavers[s] = 0; c->h_strays[s] = 0; c->h_ovf[s] = 0; }
     *ctx = c;
     return ECSIM_OK;
 }
@@ -226,12 +239,9 @@ extern "C" int ecsim_destroy(ecsim_ctx* c)
     }
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
-    for (int k = 0; k < ECSIM_MAX_SLABS; ++k)
-        if (c->ev_slab[k]) cudaEventDestroy(c->ev_slab[k]);
-    if (c->ev_aux_done) cudaEventDestroy(c->ev_aux_done);
-    if (c->aux) cudaStreamDestroy(c->aux);
     if (c->h_leavers) cudaFreeHost(c->h_leavers);
     if (c->h_strays) cudaFreeHost(c->h_strays);
+    if (c->h_ovf) cudaFreeHost(c->h_ovf);
     delete c;
     return ECSIM_OK;
 }
@@ -297,6 +307,40 @@ extern "C" int ecsim_load_particles(ecsim_ctx* c, int s, int64_t n, double q_ove
     sp.nearly_sorted = sorted != 0;
     sp.stray_debt = 0.0;
     sp.leavers_pending = false;
+    sp.res.on = false;              // a fresh load is a borrowed (dense) species again
+    return ECSIM_OK;
+}
+
+static int scan_u32(ecsim_ctx* c, const uint32_t* in, uint32_t* out /* [m+1] */, uint32_t m)
+{
+    Workspace& w = c->ws;
+    const uint32_t nb = (m + SCAN_BLOCK - 1) / SCAN_BLOCK;
+    k_scan_blocks<<<nb, SCAN_BLOCK, 0, c->stream>>>(in, out, w.block_sums, m);
+    CK_LAUNCH();
+    k_scan_sums<<<1, SCAN_BLOCK, 0, c->stream>>>(w.block_sums, nb, out, m);
+    CK_LAUNCH();
+    k_scan_add<<<nb, SCAN_BLOCK, 0, c->stream>>>(out, w.block_sums, m);
+    CK_LAUNCH();
+    c->launches += 3;
+    return ECSIM_OK;
+}
+
+// histogram of n particles at (x,y,z) -> ws.count (+ ws.cell / ws.rank)
+static int histogram(ecsim_ctx* c, uint32_t n, const double* x, const double* y, const double* z, bool with_rank)
+{
+    Workspace& w = c->ws;
+    const uint32_t cells = (uint32_t)c->g.nodes;
+    CK(cudaMemsetAsync(w.count, 0, sizeof(uint32_t) * cells, c->stream));
+    c->launches++;
+    if (n > 0) {
+        const int grid = grid_for(c, (size_t)n, 256, 16);
+        if (with_rank)
+            k_cell_hist<true><<<grid, 256, 0, c->stream>>>(c->g, n, x, y, z, w.cell, w.rank, w.count);
+        else
+            k_cell_hist<false><<<grid, 256, 0, c->stream>>>(c->g, n, x, y, z, nullptr, nullptr, w.count);
+        CK_LAUNCH();
+        c->launches++;
+    }
     return ECSIM_OK;
 }
 
@@ -304,35 +348,17 @@ extern "C" int ecsim_load_particles(ecsim_ctx* c, int s, int64_t n, double q_ove
 static int histogram_and_scan(ecsim_ctx* c, int s, bool with_rank)
 {
     SpeciesHost& sp = c->sp[s];
-    Workspace& w = c->ws;
     const uint32_t cells = (uint32_t)c->g.nodes;
-    uint32_t* start = w.start + (size_t)s * (cells + 1);
-    CK(cudaMemsetAsync(w.count, 0, sizeof(uint32_t) * cells, c->stream));
-    c->launches++;
-    if (sp.n > 0) {
-        const int grid = grid_for(c, (size_t)sp.n, 256, 16);
-        if (with_rank)
-            k_cell_hist<true><<<grid, 256, 0, c->stream>>>(c->g, (uint32_t)sp.n, sp.x, sp.y, sp.z, w.cell, w.rank, w.count);
-        else
-            k_cell_hist<false><<<grid, 256, 0, c->stream>>>(c->g, (uint32_t)sp.n, sp.x, sp.y, sp.z, nullptr, nullptr, w.count);
-        CK_LAUNCH();
-        c->launches++;
-    }
-    const uint32_t nb = (cells + SCAN_BLOCK - 1) / SCAN_BLOCK;
-    k_scan_blocks<<<nb, SCAN_BLOCK, 0, c->stream>>>(w.count, start, w.block_sums, cells);
-    CK_LAUNCH();
-    k_scan_sums<<<1, SCAN_BLOCK, 0, c->stream>>>(w.block_sums, nb, start, cells);
-    CK_LAUNCH();
-    k_scan_add<<<nb, SCAN_BLOCK, 0, c->stream>>>(start, w.block_sums, cells);
-    CK_LAUNCH();
-    c->launches += 3;
-    return ECSIM_OK;
+    int rc = histogram(c, (uint32_t)sp.n, sp.x, sp.y, sp.z, with_rank);
+    if (rc) return rc;
+    return scan_u32(c, c->ws.count, c->ws.start + (size_t)s * (cells + 1), cells);
 }
 
 extern "C" int ecsim_build_segments(ecsim_ctx* c, int s)
 {
     int rc = check_species(c, s);
     if (rc) return rc;
+    if (c->sp[s].res.on) return ECSIM_OK;          // a resident species is always segmented
     rc = need_workspace(c, c->sp[s].n);
     if (rc) return rc;
     rc = histogram_and_scan(c, s, false);
@@ -342,11 +368,14 @@ extern "C" int ecsim_build_segments(ecsim_ctx* c, int s)
     return ECSIM_OK;
 }
 
+static int resident_layout_from_dense(ecsim_ctx* c, int s, const double* const src[7], int dst_buf);
+
 extern "C" int ecsim_sort_particles(ecsim_ctx* c, int s, int32_t* cell_count_out, uint32_t* perm_out)
 {
     int rc = check_species(c, s);
     if (rc) return rc;
     SpeciesHost& sp = c->sp[s];
+    if (sp.res.on) return ECSIM_ERR_INVALID_ARG;   // resident species keep themselves sorted
     rc = need_workspace(c, sp.n);
     if (rc) return rc;
     Workspace& w = c->ws;
@@ -373,11 +402,7 @@ extern "C" int ecsim_sort_particles(ecsim_ctx* c, int s, int32_t* cell_count_out
                 CK(cudaMemcpyAsync(perm_out, w.perm, sizeof(uint32_t) * (size_t)n, cudaMemcpyDeviceToDevice, c->stream));
         } else {
             // arbitrary order: the bucketed two-step move of sort.cuh
-            static bool configured = false;
-            if (!configured) {
-                CK(cudaFuncSetAttribute(k_stage_to_slots, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SORT_STAGE_SMEM));
-                configured = true;
-            }
+            CK(cudaFuncSetAttribute(k_stage_to_slots, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SORT_STAGE_SMEM));
             int shift = 13;
             while ((((n - 1) >> shift) + 1) > (uint32_t)SORT_MAX_BUCKETS) ++shift;
             const uint32_t nbk = ((n - 1) >> shift) + 1;
@@ -429,7 +454,7 @@ extern "C" int ecsim_cell_index(ecsim_ctx* c, int s, int32_t* cell_out)
 {
     int rc = check_species(c, s);
     if (rc) return rc;
-    if (!cell_out) return ECSIM_ERR_INVALID_ARG;
+    if (!cell_out || c->sp[s].res.on) return ECSIM_ERR_INVALID_ARG;
     SpeciesHost& sp = c->sp[s];
     if (sp.n == 0) return ECSIM_OK;
     k_cell_index<<<grid_for(c, (size_t)sp.n, 256, 16), 256, 0, c->stream>>>(c->g, (uint32_t)sp.n, sp.x, sp.y, sp.z, cell_out);
@@ -438,6 +463,196 @@ extern "C" int ecsim_cell_index(ecsim_ctx* c, int s, int32_t* cell_out)
     return ECSIM_OK;
 }
 
+// --------------------------------------------------------------------------------------------
+// Resident species: library-managed gapped double buffers, sort-preserving push.
+static size_t resident_tables_bytes(const ecsim_ctx* c, uint32_t ovf_cap)
+{
+    const size_t cells = (size_t)c->g.nodes;
+    return align_up(sizeof(uint32_t) * (cells + 1), 256) + 4 * align_up(sizeof(uint32_t) * cells, 256) + 256 +
+           align_up(sizeof(double) * 7 * (size_t)ovf_cap, 256);
+}
+
+static uint32_t resident_ovf_cap(int64_t n)
+{
+    int64_t v = n / 8;
+    if (v < 65536) v = 65536;
+    return (uint32_t)v;
+}
+
+static const uint32_t RESIDENT_MIN_SLACK = 8;
+
+extern "C" size_t ecsim_resident_bytes(const ecsim_ctx* c, int64_t n, double slack)
+{
+    if (!c || n < 0 || !(slack >= 0.0) || slack > 4.0) return 0;
+    const size_t cells = (size_t)c->g.nodes;
+    // slots: n + ceil(slack n_c) per cell + the minimum slack and the rounding to 4 per cell
+    const size_t slots = (size_t)n + (size_t)ceil(slack * (double)n) + (RESIDENT_MIN_SLACK + 4) * cells + 64;
+    return resident_tables_bytes(c, resident_ovf_cap(n)) + 14 * align_up(sizeof(double) * slots, 256);
+}
+
+// Bin the dense arrays src (n = sp.n particles, any order) and lay them out, gapped, in buffer dst_buf.
+// Synchronises the stream once (the number of slots the layout needs is data dependent and is checked on the host).
+static int resident_layout_from_dense(ecsim_ctx* c, int s, const double* const src[7], int dst_buf)
+{
+    SpeciesHost& sp = c->sp[s];
+    Resident& r = sp.res;
+    Workspace& w = c->ws;
+    const uint32_t cells = (uint32_t)c->g.nodes;
+    const uint32_t n = (uint32_t)sp.n;
+    int rc = histogram(c, n, src[0], src[1], src[2], true);
+    if (rc) return rc;
+    const int cgrid = (int)((cells + 255) / 256);
+    uint32_t* cap = r.R[dst_buf];              // scratch until the runs are written
+    k_gapped_caps<<<cgrid, 256, 0, c->stream>>>(cells, w.count, r.slack, RESIDENT_MIN_SLACK, cap);
+    CK_LAUNCH();
+    c->launches++;
+    rc = scan_u32(c, cap, r.seg, cells);
+    if (rc) return rc;
+    uint32_t total = 0;
+    CK(cudaMemcpyAsync(&total, r.seg + cells, sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    if (total > r.cap_bound) return ECSIM_ERR_WORKSPACE;
+    if (n > 0) {
+        Soa7c in; Soa7 out;
+        for (int k = 0; k < 7; ++k) { in.a[k] = src[k]; out.a[k] = r.buf[dst_buf][k]; }
+        k_scatter_gapped<<<grid_for(c, (size_t)n, 256, 16), 256, 0, c->stream>>>(n, w.cell, w.rank, r.seg, in, out);
+        CK_LAUNCH();
+        c->launches++;
+    }
+    k_runs_from_count<<<cgrid, 256, 0, c->stream>>>(cells, w.count, r.F[dst_buf], r.R[dst_buf]);
+    CK_LAUNCH();
+    c->launches++;
+    r.cur = dst_buf;
+    return ECSIM_OK;
+}
+
+// gapped buffer `cur` -> dense cell-ordered arrays dst[7] (+ the overflow list of the last push behind them)
+static int resident_export(ecsim_ctx* c, int s, double* const dst[7], bool with_overflow)
+{
+    SpeciesHost& sp = c->sp[s];
+    Resident& r = sp.res;
+    Workspace& w = c->ws;
+    const uint32_t cells = (uint32_t)c->g.nodes;
+    const int cgrid = (int)((cells + 255) / 256);
+    uint32_t* start = w.start + (size_t)s * (cells + 1);   // dense start tables are not used by a resident species
+    k_run_totals<<<cgrid, 256, 0, c->stream>>>(cells, r.F[r.cur], r.R[r.cur], w.count);
+    CK_LAUNCH();
+    c->launches++;
+    int rc = scan_u32(c, w.count, start, cells);
+    if (rc) return rc;
+    Soa7c in; Soa7 out;
+    for (int k = 0; k < 7; ++k) { in.a[k] = r.buf[r.cur][k]; out.a[k] = dst[k]; }
+    k_export_gapped<<<c->sm_count * 8, 256, 0, c->stream>>>(cells, r.seg, r.F[r.cur], r.R[r.cur], start, in, out);
+    CK_LAUNCH();
+    c->launches++;
+    if (with_overflow) {
+        k_append_overflow<<<c->sm_count, 256, 0, c->stream>>>(r.ovf_count, r.ovf_cap, r.ovf, start + cells, out);
+        CK_LAUNCH();
+        c->launches++;
+    }
+    return ECSIM_OK;
+}
+
+// a push found segments full: export everything (+ the overflow list) to the idle buffer, lay out afresh
+static int resident_relayout(ecsim_ctx* c, int s)
+{
+    Resident& r = c->sp[s].res;
+    const int other = 1 - r.cur;
+    int rc = resident_export(c, s, r.buf[other], true);
+    if (rc) return rc;
+    const double* src[7];
+    for (int k = 0; k < 7; ++k) src[k] = r.buf[other][k];
+    rc = resident_layout_from_dense(c, s, src, r.cur);
+    if (rc) return rc;
+    CK(cudaMemsetAsync(r.ovf_count, 0, sizeof(uint32_t), c->stream));
+    c->relayouts++;
+    return ECSIM_OK;
+}
+
+extern "C" int ecsim_make_resident(ecsim_ctx* c, int s, void* dev_buf, size_t bytes, double slack)
+{
+    int rc = check_species(c, s);
+    if (rc) return rc;
+    if (!dev_buf || (reinterpret_cast<uintptr_t>(dev_buf) & 255u) || !(slack >= 0.0) || slack > 4.0)
+        return ECSIM_ERR_INVALID_ARG;
+    SpeciesHost& sp = c->sp[s];
+    rc = need_workspace(c, sp.n);
+    if (rc) return rc;
+    const size_t cells = (size_t)c->g.nodes;
+    Resident r;
+    r.slack = slack;
+    r.ovf_cap = resident_ovf_cap(sp.n);
+    const size_t tables = resident_tables_bytes(c, r.ovf_cap);
+    if (bytes < tables + 14 * 256) return ECSIM_ERR_WORKSPACE;
+    Carver k{reinterpret_cast<char*>(dev_buf)};
+    r.seg = k.take<uint32_t>(cells + 1);
+    r.F[0] = k.take<uint32_t>(cells); r.F[1] = k.take<uint32_t>(cells);
+    r.R[0] = k.take<uint32_t>(cells); r.R[1] = k.take<uint32_t>(cells);
+    r.ovf_count = k.take<uint32_t>(1);
+    r.ovf = k.take<double>(7 * (size_t)r.ovf_cap);
+    const size_t per_array = ((bytes - k.off) / 14) & ~(size_t)255;
+    size_t slots = per_array / sizeof(double);
+    if (slots > 0xfffffff0u) slots = 0xfffffff0u;
+    r.cap_bound = (uint32_t)slots;
+    for (int b = 0; b < 2; ++b)
+        for (int a = 0; a < 7; ++a) r.buf[b][a] = reinterpret_cast<double*>(k.p + k.off + ((size_t)b * 7 + a) * per_array);
+    if (sp.state == ST_UNSORTED && !sp.nearly_sorted && sp.n > 0) {
+        // arbitrary order: the bucketed sort first, so that the scatter into the gapped layout is sequential
+        rc = ecsim_sort_particles(c, s, nullptr, nullptr);
+        if (rc) return rc;
+    }
+    sp.res = r;
+    const double* src[7] = {sp.x, sp.y, sp.z, sp.u, sp.v, sp.w, sp.q};
+    rc = resident_layout_from_dense(c, s, src, 0);
+    if (rc) return rc;
+    CK(cudaMemsetAsync(sp.res.ovf_count, 0, sizeof(uint32_t), c->stream));
+    sp.res.on = true;
+    sp.state = ST_SEGMENTED;
+    sp.leavers_pending = false;
+    sp.stray_debt = 0.0;
+    c->h_ovf[s] = 0;
+    return ECSIM_OK;
+}
+
+// Before a call touches a resident species: the overflow counter of its last push (host-visible once that push has
+// finished) decides whether the species must be laid out afresh.
+static int resident_settle(ecsim_ctx* c, int s)
+{
+    SpeciesHost& sp = c->sp[s];
+    if (!sp.res.on || !sp.leavers_pending) return ECSIM_OK;
+    CK(cudaEventSynchronize(sp.leavers_event));
+    sp.leavers_pending = false;
+    if (c->h_ovf[s] > sp.res.ovf_cap) return ECSIM_ERR_OVERFLOW;
+    if (c->h_ovf[s] > 0) {
+        c->h_ovf[s] = 0;
+        return resident_relayout(c, s);
+    }
+    return ECSIM_OK;
+}
+
+extern "C" int ecsim_export_particles(ecsim_ctx* c, int s, double* x, double* y, double* z, double* u, double* v,
+                                      double* w, double* q)
+{
+    int rc = check_species(c, s);
+    if (rc) return rc;
+    SpeciesHost& sp = c->sp[s];
+    if (sp.n > 0 && (!x || !y || !z || !u || !v || !w || !q)) return ECSIM_ERR_INVALID_ARG;
+    double* dst[7] = {x, y, z, u, v, w, q};
+    if (!sp.res.on) {
+        double* src[7] = {sp.x, sp.y, sp.z, sp.u, sp.v, sp.w, sp.q};
+        for (int k = 0; k < 7; ++k)
+            if (dst[k] != src[k])
+                CK(cudaMemcpyAsync(dst[k], src[k], sizeof(double) * (size_t)sp.n, cudaMemcpyDeviceToDevice, c->stream));
+        return ECSIM_OK;
+    }
+    rc = resident_settle(c, s);
+    if (rc) return rc;
+    return resident_export(c, s, dst, false);
+}
+
+extern "C" int64_t ecsim_relayout_count(const ecsim_ctx* c) { return c ? c->relayouts : 0; }
+
+// --------------------------------------------------------------------------------------------
 extern "C" int ecsim_set_variant(ecsim_ctx* c, int variant)
 {
     if (!c || (variant != ECSIM_VARIANT_ATOMIC && variant != ECSIM_VARIANT_FUSED)) return ECSIM_ERR_INVALID_ARG;
@@ -459,10 +674,10 @@ extern "C" int ecsim_set_fused_warps(ecsim_ctx* c, int warps)
     return ECSIM_OK;
 }
 
-extern "C" int ecsim_set_slabs(ecsim_ctx* c, int slabs)
+extern "C" int ecsim_set_m_layout(ecsim_ctx* c, int layout)
 {
-    if (!c || slabs < 0 || slabs > ECSIM_MAX_SLABS) return ECSIM_ERR_INVALID_ARG;
-    c->slabs = slabs;
+    if (!c || (layout != ECSIM_M_27 && layout != ECSIM_M_14)) return ECSIM_ERR_INVALID_ARG;
+    c->m_layout = layout;
     return ECSIM_OK;
 }
 
@@ -495,81 +710,57 @@ extern "C" int64_t ecsim_stray_count(ecsim_ctx* c)
     return total;
 }
 
-template <int NW, int REGS>
+extern "C" int64_t ecsim_leaver_count(ecsim_ctx* c)
+{
+    if (!c || !c->ws.base || c->last_call_n == 0) return 0;
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return -1;
+    int64_t total = 0;
+    for (int i = 0; i < c->last_call_n; ++i) total += (int64_t)c->h_leavers[c->last_call_species[i]];
+    return total;
+}
+
+template <int NW, int REGS, int MODE, int LAYOUT>
 static cudaError_t launch_fused(const ecsim_ctx* c, const FusedArgs& fa)
 {
-    const size_t smem = (size_t)NW * WARP_SMEM_DOUBLES * sizeof(double);
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_fused_push_moments<NW, REGS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    const size_t smem = (size_t)NW * (MODE == MODE_PUSH ? FLD_DOUBLES : WARP_SMEM_DOUBLES) * sizeof(double);
+    // per launch, not per process: a second device of the same process needs its own opt-in
+    cudaError_t e = cudaFuncSetAttribute(k_fused_push_moments<NW, REGS, MODE, LAYOUT>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
     const size_t cells = (size_t)(fa.c_end - fa.c_begin);
     size_t grid = (cells + NW - 1) / NW;
     if (grid > (size_t)c->sm_count) grid = (size_t)c->sm_count;
-    k_fused_push_moments<NW, REGS><<<(int)grid, NW * 32, smem, c->stream>>>(fa);
+    k_fused_push_moments<NW, REGS, MODE, LAYOUT><<<(int)grid, NW * 32, smem, c->stream>>>(fa);
     return cudaGetLastError();
 }
 
-// One hot-path step for the listed species.  rho/J: per listed species (stride given), M shared.
-static int push_and_moments_impl(ecsim_ctx* c, int n_list, const int* list, const double* E, const double* B,
-                                 double dt, double theta, double* rho, size_t rho_stride, double* J,
-                                 size_t J_stride, double* M, int accumulate)
+static cudaError_t launch_fused_any(const ecsim_ctx* c, const FusedArgs& fa, int mode, bool gapped)
 {
-    if (!c || !E || !B || !(dt > 0.0) || !(theta >= 0.5 && theta <= 1.0)) return ECSIM_ERR_INVALID_ARG;
-    for (int i = 0; i < n_list; ++i) {
-        int rc = check_species(c, list[i]);
-        if (rc) return rc;
-    }
-    if (accumulate < 0 || accumulate > 2) return ECSIM_ERR_INVALID_ARG;
-    const int acc_M = accumulate != ECSIM_ACC_NONE;      // M: summed over species (L59)
-    const int acc_J = accumulate == ECSIM_ACC_ALL;       // rho/Jhat: per species unless asked (L129)
-    const Geom& g = c->g;
-    const size_t nodes = (size_t)g.nodes;
-    c->last_call_n = 0;
+    if (mode == MODE_DIAG)
+        return gapped ? launch_fused<16, 128, MODE_DIAG, LAYOUT_GAPPED>(c, fa) : launch_fused<16, 128, MODE_DIAG, LAYOUT_DENSE>(c, fa);
+    if (mode == MODE_PUSH)
+        return gapped ? launch_fused<16, 128, MODE_PUSH, LAYOUT_GAPPED>(c, fa) : launch_fused<16, 128, MODE_PUSH, LAYOUT_DENSE>(c, fa);
+    if (mode == MODE_MOMENTS)
+        return gapped ? launch_fused<12, 168, MODE_MOMENTS, LAYOUT_GAPPED>(c, fa) : launch_fused<12, 168, MODE_MOMENTS, LAYOUT_DENSE>(c, fa);
+    if (gapped) return launch_fused<12, 168, MODE_FUSED, LAYOUT_GAPPED>(c, fa);
+    if (c->fused_warps == 8) return launch_fused<8, 224, MODE_FUSED, LAYOUT_DENSE>(c, fa);
+    if (c->fused_warps == 16) return launch_fused<16, 128, MODE_FUSED, LAYOUT_DENSE>(c, fa);
+    return launch_fused<12, 168, MODE_FUSED, LAYOUT_DENSE>(c, fa);
+}
 
-    if (c->variant == ECSIM_VARIANT_ATOMIC) {
-        // the paper's design: zero the outputs, then one global atomic per scalar contribution
-        if (M && !acc_M) { CK(cudaMemsetAsync(M, 0, sizeof(double) * nodes * 243, c->stream)); c->launches++; }
-        if (!acc_J) {
-            for (int i = 0; i < n_list; ++i) {
-                if (rho) { CK(cudaMemsetAsync(rho + i * rho_stride, 0, sizeof(double) * nodes, c->stream)); c->launches++; }
-                if (J) { CK(cudaMemsetAsync(J + i * J_stride, 0, sizeof(double) * 3 * nodes, c->stream)); c->launches++; }
-            }
-        }
-        if (c->timing) CK(cudaEventRecord(c->ev0, c->stream));
-        for (int i = 0; i < n_list; ++i) {
-            SpeciesHost& sp = c->sp[list[i]];
-            if (sp.n == 0) continue;
-            AtomicArgs a;
-            a.g = g; a.n = (uint32_t)sp.n; a.list = nullptr; a.list_count = nullptr;
-            a.x = sp.x; a.y = sp.y; a.z = sp.z; a.u = sp.u; a.v = sp.v; a.w = sp.w; a.q = sp.q;
-            a.E = E; a.B = B; a.beta = sp.qom * dt / 2.0; a.dt = dt;
-            a.rho = rho ? rho + i * rho_stride : nullptr;
-            a.J = J ? J + i * J_stride : nullptr;
-            a.M = M; a.leavers = nullptr;
-            k_push_moments_atomic<false><<<grid_for(c, (size_t)sp.n, 128, 16), 128, 0, c->stream>>>(a);
-            CK_LAUNCH();
-            c->launches++;
-            sp.state = ST_UNSORTED;
-        }
-        if (c->timing) { CK(cudaEventRecord(c->ev1, c->stream)); c->ev_valid = true; }
-        return ECSIM_OK;
-    }
-
-    // ---- fused variant ----
-    int64_t n_need = 0;
-    for (int i = 0; i < n_list; ++i) n_need = c->sp[list[i]].n > n_need ? c->sp[list[i]].n : n_need;
-    int rc = need_workspace(c, n_need);
-    if (rc) return rc;
-    Workspace& w = c->ws;
-    const uint32_t cells = (uint32_t)nodes;
-
-    // segment tables: build, or re-sort when too many particles left their cell in the last push
+// Before a pass over the listed species: segment tables (build, or re-sort when too many particles left their cell in
+// the last push); resident species: a fresh layout if the last push overflowed.
+static int prepare_species(ecsim_ctx* c, int n_list, const int* list, bool gapped)
+{
+    int rc = ECSIM_OK;
     for (int i = 0; i < n_list; ++i) {
         const int s = list[i];
         SpeciesHost& sp = c->sp[s];
+        if (gapped) {
+            rc = resident_settle(c, s);
+            if (rc) return rc;
+            continue;
+        }
         if (sp.state == ST_SEGMENTED && sp.leavers_pending) {
             CK(cudaEventSynchronize(sp.leavers_event));
             sp.leavers_pending = false;
@@ -586,132 +777,191 @@ static int push_and_moments_impl(ecsim_ctx* c, int n_list, const int* list, cons
         }
         if (rc) return rc;
     }
-
+    Workspace& w = c->ws;
     CK(cudaMemsetAsync(w.stray_count, 0, sizeof(uint32_t) * c->n_species, c->stream));
     CK(cudaMemsetAsync(w.leavers, 0, sizeof(unsigned long long) * c->n_species, c->stream));
     c->launches += 2;
+    return ECSIM_OK;
+}
 
-    FusedArgs fa;
-    fa.g = g; fa.n_species = n_list; fa.E = E; fa.B = B; fa.dt = dt; fa.AM = w.AM;
+static int fill_fused_args(ecsim_ctx* c, FusedArgs& fa, int n_list, const int* list, const double* E, const double* B,
+                           double dt, bool gapped, bool push)
+{
+    Workspace& w = c->ws;
+    const uint32_t cells = (uint32_t)c->g.nodes;
+    memset(&fa, 0, sizeof(fa));
+    fa.g = c->g; fa.n_species = n_list; fa.E = E; fa.B = B; fa.dt = dt; fa.AM = w.AM;
+    fa.c_begin = 0; fa.c_end = cells;
     for (int i = 0; i < n_list; ++i) {
         const int s = list[i];
         SpeciesHost& sp = c->sp[s];
         SpeciesDev& d = fa.sp[i];
-        d.start = w.start + (size_t)s * (cells + 1);
-        d.x = sp.x; d.y = sp.y; d.z = sp.z; d.u = sp.u; d.v = sp.v; d.w = sp.w; d.q = sp.q;
         d.beta = sp.qom * dt / 2.0;
         d.n = (uint32_t)sp.n;
         d.AJ = w.AJ + (size_t)s * cells * AJ_PER_CELL;
         d.stray_list = w.stray_list + (size_t)s * (size_t)w.n_max;
         d.stray_count = w.stray_count + s;
         d.leavers = w.leavers + s;
+        if (gapped) {
+            Resident& r = sp.res;
+            double* const* in = r.buf[r.cur];
+            double* const* out = r.buf[1 - r.cur];
+            d.seg = r.seg; d.Fin = r.F[r.cur]; d.Rin = r.R[r.cur]; d.Fout = r.F[1 - r.cur]; d.Rout = r.R[1 - r.cur];
+            d.x = in[0]; d.y = in[1]; d.z = in[2]; d.u = in[3]; d.v = in[4]; d.w = in[5]; d.q = in[6];
+            d.ox = out[0]; d.oy = out[1]; d.oz = out[2]; d.ou = out[3]; d.ov = out[4]; d.ow = out[5]; d.oq = out[6];
+            d.ovf = r.ovf; d.ovf_cap = r.ovf_cap; d.ovf_count = r.ovf_count;
+            if (push) {
+                CK(cudaMemsetAsync(d.Rout, 0, sizeof(uint32_t) * cells, c->stream));
+                c->launches++;
+            }
+        } else {
+            d.seg = w.start + (size_t)s * (cells + 1);
+            d.x = sp.x; d.y = sp.y; d.z = sp.z; d.u = sp.u; d.v = sp.v; d.w = sp.w; d.q = sp.q;
+        }
+    }
+    return ECSIM_OK;
+}
+
+// One pass of the hot path for the listed species.  mode: MODE_FUSED (deposit + push), MODE_MOMENTS (deposit only),
+// MODE_PUSH (push only).  rho/J: per listed species (stride given), M shared.
+static int step_impl(ecsim_ctx* c, int mode, int n_list, const int* list, const double* E, const double* B,
+                     double dt, double theta, double* rho, size_t rho_stride, double* J, size_t J_stride, double* M,
+                     int accumulate)
+{
+    const bool deposit = mode != MODE_PUSH, push = mode != MODE_MOMENTS;
+    if (!c || !B || (push && !E) || !(dt > 0.0) || !(theta >= 0.5 && theta <= 1.0)) return ECSIM_ERR_INVALID_ARG;
+    for (int i = 0; i < n_list; ++i) {
+        int rc = check_species(c, list[i]);
+        if (rc) return rc;
+    }
+    if (accumulate < 0 || accumulate > 2) return ECSIM_ERR_INVALID_ARG;
+    const int acc_M = accumulate != ECSIM_ACC_NONE;      // M: summed over species (L59)
+    const int acc_J = accumulate == ECSIM_ACC_ALL;       // rho/Jhat: per species unless asked (L129)
+    const Geom& g = c->g;
+    const size_t nodes = (size_t)g.nodes;
+    c->last_call_n = 0;
+    int n_resident = 0;
+    for (int i = 0; i < n_list; ++i) n_resident += c->sp[list[i]].res.on ? 1 : 0;
+    if (n_resident != 0 && n_resident != n_list) return ECSIM_ERR_INVALID_ARG;   // one layout per call
+    const bool gapped = n_resident > 0;
+
+    if (c->variant == ECSIM_VARIANT_ATOMIC) {
+        // the paper's design: zero the outputs, then one global atomic per scalar contribution
+        if (gapped || c->m_layout != ECSIM_M_27) return ECSIM_ERR_INVALID_ARG;
+        if (deposit) {
+            if (M && !acc_M) { CK(cudaMemsetAsync(M, 0, sizeof(double) * nodes * 243, c->stream)); c->launches++; }
+            if (!acc_J) {
+                for (int i = 0; i < n_list; ++i) {
+                    if (rho) { CK(cudaMemsetAsync(rho + i * rho_stride, 0, sizeof(double) * nodes, c->stream)); c->launches++; }
+                    if (J) { CK(cudaMemsetAsync(J + i * J_stride, 0, sizeof(double) * 3 * nodes, c->stream)); c->launches++; }
+                }
+            }
+        }
+        if (c->timing) CK(cudaEventRecord(c->ev0, c->stream));
+        for (int i = 0; i < n_list; ++i) {
+            SpeciesHost& sp = c->sp[list[i]];
+            if (sp.n == 0) continue;
+            AtomicArgs a;
+            a.g = g; a.n = (uint32_t)sp.n; a.list = nullptr; a.list_count = nullptr;
+            a.x = sp.x; a.y = sp.y; a.z = sp.z; a.u = sp.u; a.v = sp.v; a.w = sp.w; a.q = sp.q;
+            a.E = push ? E : B;            // moments only: E is not used by the deposit (any valid pointer)
+            a.B = B; a.beta = sp.qom * dt / 2.0; a.dt = dt;
+            a.rho = (deposit && rho) ? rho + i * rho_stride : nullptr;
+            a.J = (deposit && J) ? J + i * J_stride : nullptr;
+            a.M = deposit ? M : nullptr; a.leavers = nullptr;
+            a.do_push = push ? 1 : 0;
+            k_push_moments_atomic<false><<<grid_for(c, (size_t)sp.n, 128, 16), 128, 0, c->stream>>>(a);
+            CK_LAUNCH();
+            c->launches++;
+            if (push) sp.state = ST_UNSORTED;
+        }
+        if (c->timing) { CK(cudaEventRecord(c->ev1, c->stream)); c->ev_valid = true; }
+        return ECSIM_OK;
     }
 
-    // Slabs of x-planes: the fused kernel of slab s (main stream) overlaps the expansion of slab s-1
-    // (aux stream): the first is bound by FP64 issue, the second by HBM.  Node plane i needs the cell
-    // planes i-1 and i, so slab s expands its own planes; plane 0 (which needs plane nx-1) goes last.
-    int n_slabs = c->slabs;
-    if (n_slabs == 0) n_slabs = 1;   // measured on config 2: 1 slab 14.4 ms, 4 slabs 15.0, 8 slabs 15.3
-    if (n_slabs > g.nx) n_slabs = g.nx;
-    const size_t plane = (size_t)g.ny * g.nz;
-    const bool overlap = n_slabs > 1;
-    auto expand_planes = [&](int i0, int i1, cudaStream_t st) -> int {
-        if (i1 <= i0) return ECSIM_OK;
-        if (M) {
-            // one short-lived CTA per (i,j) column (persistent CTAs kept the next slab's fused launch waiting)
-            ExpandStreamArgs ea{g, w.AM, M, acc_M, i0, i1};
-            k_expand_M_stream<<<(i1 - i0) * g.ny, XS_THREADS, XS_SMEM_BYTES, st>>>(ea);
-            CK_LAUNCH();
-            c->launches++;
-        }
-        for (int i = 0; i < n_list && (rho || J); ++i) {
-            ExpandJArgs ja{g, fa.sp[i].AJ, rho ? rho + i * rho_stride : nullptr, J ? J + i * J_stride : nullptr, acc_J,
-                           (long long)(i0 * plane), (long long)(i1 * plane)};
-            k_expand_rhoJ<<<(unsigned)(((size_t)(i1 - i0) * plane + 255) / 256), 256, 0, st>>>(ja);
-            CK_LAUNCH();
-            c->launches++;
-        }
-        return ECSIM_OK;
-    };
-    // With slabs (ecsim_set_slabs > 1) the fused kernels stay on the caller's stream as 12 warps x 144 registers,
-    // and the expansions go to the context's second stream: one 128-thread expansion CTA fits beside a fused CTA
-    // on every SM.  Measured on config 2 this overlap does not pay (1 slab 14.4 ms, 4 slabs 15.0, 8 slabs 15.3:
-    // the fused kernel needs every warp slot and register of the SM, so the expansion beside it is not free, and it
-    // loses its 168-register schedule); the default is one slab.  Other measured alternatives, all slower: fused
-    // kernels on a high-priority stream with 8-24 SMs left free; persistent expansion CTAs.
-    const int warps = c->fused_warps;
+    // ---- fused variant ----
+    int64_t n_need = 0;
+    for (int i = 0; i < n_list; ++i) n_need = c->sp[list[i]].n > n_need ? c->sp[list[i]].n : n_need;
+    int rc = need_workspace(c, n_need);
+    if (rc) return rc;
+    Workspace& w = c->ws;
+
+    rc = prepare_species(c, n_list, list, gapped);
+    if (rc) return rc;
+    FusedArgs fa;
+    rc = fill_fused_args(c, fa, n_list, list, push ? E : B, B, dt, gapped, push);
+    if (rc) return rc;
+
     if (c->timing) CK(cudaEventRecord(c->ev0, c->stream));
-    for (int sl = 0; sl < n_slabs; ++sl) {
-        const int i0 = (int)((long long)g.nx * sl / n_slabs), i1 = (int)((long long)g.nx * (sl + 1) / n_slabs);
-        fa.c_begin = (uint32_t)(i0 * plane);
-        fa.c_end = (uint32_t)(i1 * plane);
-        cudaError_t e;
-        if (overlap) e = launch_fused<12, ECPUSH_OVERLAP_REGS>(c, fa);
-        else if (warps == 8) e = launch_fused<8, 224>(c, fa);
-        else if (warps == 16) e = launch_fused<16, 128>(c, fa);
-        else e = launch_fused<12, 168>(c, fa);
+    {
+        cudaError_t e = launch_fused_any(c, fa, mode, gapped);
         if (e != cudaSuccess) return cuda_fail(e, "k_fused_push_moments launch", __LINE__);
         c->launches++;
-        if (overlap) {
-            CK(cudaEventRecord(c->ev_slab[sl], c->stream));
-            CK(cudaStreamWaitEvent(c->aux, c->ev_slab[sl], 0));
-            rc = expand_planes(sl == 0 ? 1 : i0, i1, c->aux);
-            if (rc) return rc;
-        }
     }
     if (c->timing) { CK(cudaEventRecord(c->ev1, c->stream)); c->ev_valid = true; }
-    if (overlap) {
-        rc = expand_planes(0, 1, c->aux);
-        if (rc) return rc;
-        CK(cudaEventRecord(c->ev_aux_done, c->aux));
-        CK(cudaStreamWaitEvent(c->stream, c->ev_aux_done, 0));
-    } else {
-        // strays first: each is added to the per-cell accumulators of its true cell with one bulk reduction (a 2.2 KB
-        // block instead of atomics on eight node blocks), then one expansion serves everybody
+
+    // strays (dense layout only): each is added to the per-cell accumulators of its true cell with one bulk reduction
+    // (a 2.2 KB block instead of atomics on eight node blocks), then one expansion serves everybody
+    if (!gapped) {
         for (int i = 0; i < n_list; ++i) {
             const SpeciesHost& sp = c->sp[list[i]];
             if (sp.n == 0) continue;
             StrayArgs a;
             a.g = g; a.list = fa.sp[i].stray_list; a.list_count = fa.sp[i].stray_count;
             a.x = sp.x; a.y = sp.y; a.z = sp.z; a.u = sp.u; a.v = sp.v; a.w = sp.w; a.q = sp.q;
-            a.E = E; a.B = B; a.beta = fa.sp[i].beta; a.dt = dt;
+            a.E = fa.E; a.B = B; a.beta = fa.sp[i].beta; a.dt = dt;
             a.AM = w.AM; a.AJ = fa.sp[i].AJ; a.leavers = fa.sp[i].leavers;
+            a.do_deposit = deposit ? 1 : 0; a.do_push = push ? 1 : 0;
             k_push_strays_bulk<<<c->sm_count * 8, STRAY_WARPS * 32, 0, c->stream>>>(a, AM_PER_CELL, AM_A8);
             CK_LAUNCH();
             c->launches++;
         }
-        rc = expand_planes(0, g.nx, c->stream);
-        if (rc) return rc;
     }
-    // with slabs the expansions have run already: the strays go to the node arrays through the atomic path
-    for (int i = 0; i < n_list; ++i) {
-        const int s = list[i];
-        SpeciesHost& sp = c->sp[s];
-        if (sp.n > 0 && overlap) {
-            AtomicArgs a;
-            a.g = g; a.n = (uint32_t)sp.n; a.list = fa.sp[i].stray_list; a.list_count = fa.sp[i].stray_count;
-            a.x = sp.x; a.y = sp.y; a.z = sp.z; a.u = sp.u; a.v = sp.v; a.w = sp.w; a.q = sp.q;
-            a.E = E; a.B = B; a.beta = fa.sp[i].beta; a.dt = dt;
-            a.rho = rho ? rho + i * rho_stride : nullptr;
-            a.J = J ? J + i * J_stride : nullptr;
-            a.M = M; a.leavers = fa.sp[i].leavers;
-            k_push_moments_atomic<true><<<c->sm_count * 2, 128, 0, c->stream>>>(a);
+    if (deposit) {
+        if (M) {
+            // one short-lived CTA per (i,j) column of nodes
+            ExpandStreamArgs ea{g, w.AM, M, acc_M, 0, g.nx};
+            if (c->m_layout == ECSIM_M_14) k_expand_M_stream<14><<<g.nx * g.ny, XS_THREADS, XS_SMEM_BYTES, c->stream>>>(ea);
+            else k_expand_M_stream<27><<<g.nx * g.ny, XS_THREADS, XS_SMEM_BYTES, c->stream>>>(ea);
             CK_LAUNCH();
             c->launches++;
         }
-        CK(cudaMemcpyAsync(c->h_leavers + s, w.leavers + s, sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+        for (int i = 0; i < n_list && (rho || J); ++i) {
+            ExpandJArgs ja{g, fa.sp[i].AJ, rho ? rho + i * rho_stride : nullptr, J ? J + i * J_stride : nullptr, acc_J,
+                           0, (long long)nodes};
+            k_expand_rhoJ<<<(unsigned)((nodes + 255) / 256), 256, 0, c->stream>>>(ja);
+            CK_LAUNCH();
+            c->launches++;
+        }
+    }
+    for (int i = 0; i < n_list; ++i) {
+        const int s = list[i];
+        SpeciesHost& sp = c->sp[s];
         CK(cudaMemcpyAsync(c->h_strays + s, w.stray_count + s, sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream));
-        CK(cudaEventRecord(sp.leavers_event, c->stream));
-        sp.leavers_pending = true;
+        if (push) {
+            CK(cudaMemcpyAsync(c->h_leavers + s, w.leavers + s, sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+            if (gapped) {
+                CK(cudaMemcpyAsync(c->h_ovf + s, sp.res.ovf_count, sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream));
+                sp.res.cur = 1 - sp.res.cur;            // the species now lives in the buffer just written
+            }
+            CK(cudaEventRecord(sp.leavers_event, c->stream));
+            sp.leavers_pending = true;
+        }
         c->last_call_species[c->last_call_n++] = s;
     }
     return ECSIM_OK;
 }
 
+static int all_species(const ecsim_ctx* c, int* list)
+{
+    for (int s = 0; s < c->n_species; ++s) list[s] = s;
+    return c->n_species;
+}
+
 extern "C" int ecsim_push_and_moments(ecsim_ctx* c, int species, const double* E_theta, const double* B,
                                       double dt, double theta, double* rho, double* Jhat, double* M, int accumulate)
 {
-    return push_and_moments_impl(c, 1, &species, E_theta, B, dt, theta, rho, 0, Jhat, 0, M, accumulate);
+    return step_impl(c, MODE_FUSED, 1, &species, E_theta, B, dt, theta, rho, 0, Jhat, 0, M, accumulate);
 }
 
 extern "C" int ecsim_push_and_moments_all(ecsim_ctx* c, const double* E_theta, const double* B, double dt,
@@ -719,13 +969,113 @@ extern "C" int ecsim_push_and_moments_all(ecsim_ctx* c, const double* E_theta, c
 {
     if (!c) return ECSIM_ERR_INVALID_ARG;
     int list[ECSIM_MAX_SPECIES];
-    for (int s = 0; s < c->n_species; ++s) list[s] = s;
+    const int n = all_species(c, list);
     const size_t nodes = (size_t)c->g.nodes;
-    return push_and_moments_impl(c, c->n_species, list, E_theta, B, dt, theta, rho, nodes, Jhat, 3 * nodes, M, accumulate);
+    return step_impl(c, MODE_FUSED, n, list, E_theta, B, dt, theta, rho, nodes, Jhat, 3 * nodes, M, accumulate);
+}
+
+extern "C" int ecsim_moments(ecsim_ctx* c, int species, const double* B, double dt, double* rho, double* Jhat,
+                             double* M, int accumulate)
+{
+    return step_impl(c, MODE_MOMENTS, 1, &species, nullptr, B, dt, 0.5, rho, 0, Jhat, 0, M, accumulate);
+}
+
+extern "C" int ecsim_moments_all(ecsim_ctx* c, const double* B, double dt, double* rho, double* Jhat, double* M,
+                                 int accumulate)
+{
+    if (!c) return ECSIM_ERR_INVALID_ARG;
+    int list[ECSIM_MAX_SPECIES];
+    const int n = all_species(c, list);
+    const size_t nodes = (size_t)c->g.nodes;
+    return step_impl(c, MODE_MOMENTS, n, list, nullptr, B, dt, 0.5, rho, nodes, Jhat, 3 * nodes, M, accumulate);
+}
+
+extern "C" int ecsim_push(ecsim_ctx* c, int species, const double* E_theta, const double* B, double dt, double theta)
+{
+    return step_impl(c, MODE_PUSH, 1, &species, E_theta, B, dt, theta, nullptr, 0, nullptr, 0, nullptr, ECSIM_ACC_NONE);
+}
+
+extern "C" int ecsim_push_all(ecsim_ctx* c, const double* E_theta, const double* B, double dt, double theta)
+{
+    if (!c) return ECSIM_ERR_INVALID_ARG;
+    int list[ECSIM_MAX_SPECIES];
+    const int n = all_species(c, list);
+    return step_impl(c, MODE_PUSH, n, list, E_theta, B, dt, theta, nullptr, 0, nullptr, 0, nullptr, ECSIM_ACC_NONE);
+}
+
+// Diagnostic moments of one species: rho [nodes], un-rotated J [3][nodes], pressure tensor
+// P [6][nodes] (xx,xy,xz,yy,yz,zz), heat flux Q [3][nodes]; any may be NULL.  Overwrites.
+extern "C" int ecsim_diagnostics(ecsim_ctx* c, int species, double* rho, double* J, double* P, double* Q)
+{
+    int rc = check_species(c, species);
+    if (rc) return rc;
+    SpeciesHost& sp = c->sp[species];
+    rc = need_workspace(c, sp.n);
+    if (rc) return rc;
+    const Geom& g = c->g;
+    const size_t nodes = (size_t)g.nodes;
+    Workspace& w = c->ws;
+    c->last_call_n = 0;
+    if (c->variant == ECSIM_VARIANT_ATOMIC && !sp.res.on) {
+        // the paper's design for these routines too (L147 "#pragma acc atomic update"): every particle through the atomic kernel
+        if (rho) CK(cudaMemsetAsync(rho, 0, sizeof(double) * nodes, c->stream));
+        if (J) CK(cudaMemsetAsync(J, 0, sizeof(double) * 3 * nodes, c->stream));
+        if (P) CK(cudaMemsetAsync(P, 0, sizeof(double) * 6 * nodes, c->stream));
+        if (Q) CK(cudaMemsetAsync(Q, 0, sizeof(double) * 3 * nodes, c->stream));
+        if (sp.n > 0) {
+            k_iota_u32<<<grid_for(c, (size_t)sp.n, 256, 16), 256, 0, c->stream>>>((uint32_t)sp.n, w.perm, w.stray_count + species);
+            CK_LAUNCH();
+            DiagStrayArgs a{g, w.perm, w.stray_count + species, sp.x, sp.y, sp.z, sp.u, sp.v, sp.w, sp.q, rho, J, P, Q};
+            k_diag_strays<<<grid_for(c, (size_t)sp.n, 128, 16), 128, 0, c->stream>>>(a);
+            CK_LAUNCH();
+            c->launches += 2;
+        }
+        return ECSIM_OK;
+    }
+    const bool gapped = sp.res.on;
+    rc = prepare_species(c, 1, &species, gapped);
+    if (rc) return rc;
+    FusedArgs fa;
+    rc = fill_fused_args(c, fa, 1, &species, nullptr, nullptr, 1.0, gapped, false);
+    if (rc) return rc;
+    fa.sp[0].AJ = w.AM;                 // the per-cell corner blocks [cells][8][16] live in the class-sum array (128 <= 244 doubles per cell)
+    cudaError_t e = launch_fused_any(c, fa, MODE_DIAG, gapped);
+    if (e != cudaSuccess) return cuda_fail(e, "k_fused_push_moments<MODE_DIAG> launch", __LINE__);
+    c->launches++;
+    ExpandDiagArgs ea{g, w.AM, rho, J, P, Q};
+    k_expand_diag<<<(unsigned)((nodes + 255) / 256), 256, 0, c->stream>>>(ea);
+    CK_LAUNCH();
+    c->launches++;
+    if (!gapped && sp.n > 0) {
+        DiagStrayArgs a{g, fa.sp[0].stray_list, fa.sp[0].stray_count, sp.x, sp.y, sp.z, sp.u, sp.v, sp.w, sp.q, rho, J, P, Q};
+        k_diag_strays<<<c->sm_count * 2, 128, 0, c->stream>>>(a);
+        CK_LAUNCH();
+        c->launches++;
+    }
+    CK(cudaMemcpyAsync(c->h_strays + species, w.stray_count + species, sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream));
+    c->last_call_species[c->last_call_n++] = species;
+    return ECSIM_OK;
+}
+
+// sum_N' M_NN' E_N' (Eq. 4-5): the operator a field solve applies; M in the context's current layout (27 or 14 slots)
+extern "C" int ecsim_apply_M(ecsim_ctx* c, const double* M, const double* E, double* out, int accumulate)
+{
+    if (!c || !M || !E || !out || E == out) return ECSIM_ERR_INVALID_ARG;
+    ApplyMArgs a{c->g, M, E, out, accumulate ? 1 : 0};
+    const size_t blocks_needed = ((size_t)c->g.nodes + APPLY_WARPS - 1) / APPLY_WARPS;
+    size_t grid = (size_t)c->sm_count * 8;
+    if (grid > blocks_needed) grid = blocks_needed;
+    if (c->m_layout == ECSIM_M_14) k_apply_M<14><<<(int)grid, APPLY_WARPS * 32, 0, c->stream>>>(a);
+    else k_apply_M<27><<<(int)grid, APPLY_WARPS * 32, 0, c->stream>>>(a);
+    CK_LAUNCH();
+    c->launches++;
+    return ECSIM_OK;
 }
 
 // --------------------------------------------------------------------------------------------
 // Host-buffer steps (the end-to-end path): stage in the workspace tail, run, copy back, synchronise.
+static size_t m_doubles_per_node(const ecsim_ctx* c) { return c->m_layout == ECSIM_M_14 ? 126 : 243; }
+
 static size_t host_step_extra(const ecsim_ctx* c, int64_t n_total, int n_species_out)
 {
     const size_t nodes = (size_t)c->g.nodes;
@@ -761,11 +1111,12 @@ static int host_step_impl(ecsim_ctx* c, int nsp, const int64_t* n, const double*
     if (!c->ws.base || c->ws.bytes < ecsim_workspace_bytes(c, n_max) + host_step_extra(c, n_total, nsp))
         return ECSIM_ERR_WORKSPACE;
     // re-carve so that exactly n_max particles are served and the tail is free for staging
-    Workspace keep = c->ws;
+    const Workspace keep = c->ws;
     const size_t used = carve(c, n_max, keep.base, &c->ws);
     c->ws.bytes = keep.bytes;
     char* tail = reinterpret_cast<char*>(keep.base) + used;
     const size_t nodes = (size_t)c->g.nodes;
+    const size_t mdoubles = m_doubles_per_node(c) * nodes;
     double* dpart = reinterpret_cast<double*>(tail);
     tail += align_up(sizeof(double) * 7 * (size_t)n_total, 256);
     double* dE = reinterpret_cast<double*>(tail);
@@ -777,36 +1128,49 @@ static int host_step_impl(ecsim_ctx* c, int nsp, const int64_t* n, const double*
     double* dM = reinterpret_cast<double*>(tail);
     cudaStream_t st = c->stream;
     SpeciesHost saved[ECSIM_MAX_SPECIES];
-    int rc = ECSIM_OK;
-    {
+    for (int s = 0; s < nsp; ++s) saved[s] = c->sp[s];
+
+    // every exit goes through `restore`: the caller's species and the full carve come back whatever happened
+    auto restore = [&]() {
+        for (int s = 0; s < nsp; ++s) {
+            cudaEvent_t ev = c->sp[s].leavers_event;
+            c->sp[s] = saved[s];
+            c->sp[s].leavers_event = ev;
+            c->sp[s].leavers_pending = false;
+        }
+        const size_t used2 = carve(c, keep.n_max, keep.base, &c->ws);
+        c->ws.bytes = keep.bytes;
+        c->ws.extra = reinterpret_cast<char*>(keep.base) + used2;
+        c->ws.extra_bytes = keep.bytes - used2;
+        for (int s = 0; s < c->n_species; ++s)
+            if (c->sp[s].state == ST_SEGMENTED && !c->sp[s].res.on) c->sp[s].state = ST_DECLARED;   // the tables lived in the re-carved buffer
+    };
+    auto body = [&]() -> int {
         double* d = dpart;
-        for (int s = 0; s < nsp && rc == ECSIM_OK; ++s) {
+        for (int s = 0; s < nsp; ++s) {
             const size_t pn = (size_t)n[s];
             double* hp[7] = {hx[s], hy[s], hz[s], hu[s], hv[s], hw[s], const_cast<double*>(hq[s])};
             for (int a = 0; a < 7; ++a)
                 CK(cudaMemcpyAsync(d + a * pn, hp[a], sizeof(double) * pn, cudaMemcpyHostToDevice, st));
-            saved[s] = c->sp[s];
-            rc = ecsim_load_particles(c, s, n[s], qom[s], d, d + pn, d + 2 * pn, d + 3 * pn, d + 4 * pn, d + 5 * pn,
-                                      d + 6 * pn, sorted);
+            int rc = ecsim_load_particles(c, s, n[s], qom[s], d, d + pn, d + 2 * pn, d + 3 * pn, d + 4 * pn, d + 5 * pn,
+                                          d + 6 * pn, sorted);
+            if (rc) return rc;
             d += 7 * pn;
         }
-    }
-    CK(cudaMemcpyAsync(dE, E_theta, sizeof(double) * 3 * nodes, cudaMemcpyHostToDevice, st));
-    CK(cudaMemcpyAsync(dB, B, sizeof(double) * 3 * nodes, cudaMemcpyHostToDevice, st));
-    if (accumulate == ECSIM_ACC_ALL) {
-        if (rho) CK(cudaMemcpyAsync(drho, rho, sizeof(double) * nodes * nsp, cudaMemcpyHostToDevice, st));
-        if (Jhat) CK(cudaMemcpyAsync(dJ, Jhat, sizeof(double) * 3 * nodes * nsp, cudaMemcpyHostToDevice, st));
-    }
-    if (accumulate != ECSIM_ACC_NONE && M)
-        CK(cudaMemcpyAsync(dM, M, sizeof(double) * 243 * nodes, cudaMemcpyHostToDevice, st));
-    if (rc == ECSIM_OK) {
+        CK(cudaMemcpyAsync(dE, E_theta, sizeof(double) * 3 * nodes, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(dB, B, sizeof(double) * 3 * nodes, cudaMemcpyHostToDevice, st));
+        if (accumulate == ECSIM_ACC_ALL) {
+            if (rho) CK(cudaMemcpyAsync(drho, rho, sizeof(double) * nodes * nsp, cudaMemcpyHostToDevice, st));
+            if (Jhat) CK(cudaMemcpyAsync(dJ, Jhat, sizeof(double) * 3 * nodes * nsp, cudaMemcpyHostToDevice, st));
+        }
+        if (accumulate != ECSIM_ACC_NONE && M)
+            CK(cudaMemcpyAsync(dM, M, sizeof(double) * mdoubles, cudaMemcpyHostToDevice, st));
         int list[ECSIM_MAX_SPECIES];
         for (int s = 0; s < nsp; ++s) list[s] = s;
-        rc = push_and_moments_impl(c, nsp, list, dE, dB, dt, theta, rho ? drho : nullptr, all_species_call ? nodes : 0,
-                                   Jhat ? dJ : nullptr, all_species_call ? 3 * nodes : 0, M ? dM : nullptr, accumulate);
-    }
-    if (rc == ECSIM_OK) {
-        double* d = dpart;
+        int rc = step_impl(c, MODE_FUSED, nsp, list, dE, dB, dt, theta, rho ? drho : nullptr, all_species_call ? nodes : 0,
+                           Jhat ? dJ : nullptr, all_species_call ? 3 * nodes : 0, M ? dM : nullptr, accumulate);
+        if (rc) return rc;
+        d = dpart;
         for (int s = 0; s < nsp; ++s) {
             const size_t pn = (size_t)n[s];
             double* hp[6] = {hx[s], hy[s], hz[s], hu[s], hv[s], hw[s]};
@@ -816,22 +1180,13 @@ static int host_step_impl(ecsim_ctx* c, int nsp, const int64_t* n, const double*
         }
         if (rho) CK(cudaMemcpyAsync(rho, drho, sizeof(double) * nodes * nsp, cudaMemcpyDeviceToHost, st));
         if (Jhat) CK(cudaMemcpyAsync(Jhat, dJ, sizeof(double) * 3 * nodes * nsp, cudaMemcpyDeviceToHost, st));
-        if (M) CK(cudaMemcpyAsync(M, dM, sizeof(double) * 243 * nodes, cudaMemcpyDeviceToHost, st));
+        if (M) CK(cudaMemcpyAsync(M, dM, sizeof(double) * mdoubles, cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
-    }
-    // restore the caller's species and the full carve
-    for (int s = 0; s < nsp; ++s) {
-        cudaEvent_t ev = c->sp[s].leavers_event;
-        c->sp[s] = saved[s];
-        c->sp[s].leavers_event = ev;
-        c->sp[s].leavers_pending = false;
-    }
-    const size_t used2 = carve(c, keep.n_max, keep.base, &c->ws);
-    c->ws.bytes = keep.bytes;
-    c->ws.extra = reinterpret_cast<char*>(keep.base) + used2;
-    c->ws.extra_bytes = keep.bytes - used2;
-    for (int s = 0; s < c->n_species; ++s)
-        if (c->sp[s].state == ST_SEGMENTED) c->sp[s].state = ST_DECLARED;   // the tables lived in the re-carved buffer
+        return ECSIM_OK;
+    };
+    const int rc = body();
+    if (rc != ECSIM_OK) cudaStreamSynchronize(st);      // nothing of the failed call may still use the staging area
+    restore();
     return rc;
 }
 

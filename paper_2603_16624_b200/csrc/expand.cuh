@@ -24,6 +24,14 @@ __device__ __constant__ unsigned char EXPAND_ORDER[27] = {
     3, 5, 9, 11, 15, 17, 21, 23,
     1, 7, 19, 25,
     0, 2, 6, 8, 18, 20, 24, 26};
+// the 14 slots o >= 13 of the symmetric storage (L73), same ordering rule
+__device__ __constant__ unsigned char EXPAND_ORDER14[14] = {
+    13,
+    14,
+    16, 22,
+    15, 17, 21, 23,
+    19, 25,
+    18, 20, 24, 26};
 
 // Offset, in doubles inside a cell's AM block, of (class, ij): 8*class + ij for ij < 8, AM_A8 + class for
 // ij = 8 -- additive in the per-axis parts of class = 9 clx + 3 cly + clz.
@@ -64,4 +72,44 @@ k_expand_rhoJ(ExpandJArgs a)
         a.J[g.nodes + node] = (a.accumulate ? a.J[g.nodes + node] : 0.0) + s2;
         a.J[2 * g.nodes + node] = (a.accumulate ? a.J[2 * g.nodes + node] : 0.0) + s3;
     }
+}
+
+// MODE_DIAG (fused_mma.cuh): node sums of the per-cell corner blocks AD[cell][8][16] -> rho, J (un-rotated), P, Q
+// (PAPER.md L121, L147).  Column c of a corner block: 0 rho; 1..3 J; 4..9 P (xx,xy,xz,yy,yz,zz); 10..12 Q.
+struct ExpandDiagArgs {
+    Geom g;
+    const double* AD;   // [cells][8][16]
+    double *rho, *J, *P, *Q;   // [nodes], [3][nodes], [6][nodes], [3][nodes]; any may be null
+};
+
+__global__ void __launch_bounds__(256)
+k_expand_diag(ExpandDiagArgs a)
+{
+    const Geom& g = a.g;
+    const long long node = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (node >= g.nodes) return;
+    const int k = (int)(node % g.nz);
+    const int j = (int)((node / g.nz) % g.ny);
+    const int i = (int)(node / ((long long)g.nz * g.ny));
+    double s[13];
+#pragma unroll
+    for (int c = 0; c < 13; ++c) s[c] = 0.0;
+#pragma unroll
+    for (int corner = 0; corner < 8; ++corner) {
+        int ci = i - ((corner >> 2) & 1); if (ci < 0) ci += g.nx;
+        int cj = j - ((corner >> 1) & 1); if (cj < 0) cj += g.ny;
+        int ck = k - (corner & 1);        if (ck < 0) ck += g.nz;
+        const long long cell = ((long long)ci * g.ny + cj) * g.nz + ck;
+        const double* src = a.AD + (size_t)cell * AD_PER_CELL + corner * 16;
+#pragma unroll
+        for (int c = 0; c < 12; c += 2) {
+            const double2 v = *reinterpret_cast<const double2*>(src + c);
+            s[c] += v.x; s[c + 1] += v.y;
+        }
+        s[12] += src[12];
+    }
+    if (a.rho) a.rho[node] = s[0];
+    if (a.J) for (int c = 0; c < 3; ++c) a.J[(size_t)c * g.nodes + node] = s[1 + c];
+    if (a.P) for (int c = 0; c < 6; ++c) a.P[(size_t)c * g.nodes + node] = s[4 + c];
+    if (a.Q) for (int c = 0; c < 3; ++c) a.Q[(size_t)c * g.nodes + node] = s[10 + c];
 }

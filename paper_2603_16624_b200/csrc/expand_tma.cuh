@@ -27,7 +27,6 @@
 #endif
 constexpr int XS_THREADS = XS_THREADS_N;
 constexpr int XS_RING = XS_RING_N;
-constexpr int XS_OUT = (243 + XS_THREADS - 1) / XS_THREADS;   // outputs per thread
 constexpr int XS_STAGE_DOUBLES = 4 * AM_PER_CELL;                       // cells (i,j), (i,j-1), (i-1,j), (i-1,j-1)
 constexpr int XS_STAGE_BYTES = XS_STAGE_DOUBLES * 8;                    // 7808
 constexpr int XS_SMEM_BYTES = XS_RING * XS_STAGE_BYTES + XS_RING * 8;   // ring + mbarriers
@@ -63,7 +62,7 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned by
 struct ExpandStreamArgs {
     Geom g;
     const double* AM;   // [cells][AM_PER_CELL]
-    double* M;          // [nodes][27][3][3]
+    double* M;          // [nodes][NSLOT][3][3]
     int accumulate;
     int i0, i1;         // node planes [i0, i1) of this launch
 };
@@ -97,9 +96,15 @@ __device__ __forceinline__ double xs_sum(double s, uint32_t offA, uint32_t offB,
 
 // One CTA per (i,j) column of nodes; stage q = 0 holds the cells at z = nz-1 (the "k-1" of node 0), stage q >= 1 the
 // cells at z = q-1; node k reads stages k ("previous level") and k+1 ("own level"); stage q lives in slot q % XS_RING.
+// NSLOT = 27: every neighbour slot (the north-star layout).  NSLOT = 14: the symmetric storage of the paper (L73, L129):
+// only the slots o >= 13 (self and the 13 "upper" neighbours) are written, M14[node][o - 13][3][3]; the others follow
+// from M[g][o] = M[g + off(o)][26 - o].
+template <int NSLOT>
 __global__ void __launch_bounds__(XS_THREADS, 1024 / XS_THREADS)   // <= 64 registers
 k_expand_M_stream(const __grid_constant__ ExpandStreamArgs a)
 {
+    constexpr int NOUT = NSLOT * 9;
+    constexpr int XS_OUT = (NOUT + XS_THREADS - 1) / XS_THREADS;   // outputs per thread
     extern __shared__ __align__(128) unsigned char xs_smem[];
     double* ring = reinterpret_cast<double*>(xs_smem);
     uint64_t* bars = reinterpret_cast<uint64_t*>(xs_smem + (size_t)XS_RING * XS_STAGE_BYTES);
@@ -133,7 +138,7 @@ k_expand_M_stream(const __grid_constant__ ExpandStreamArgs a)
     if (tid == 0)
         for (int s = 0; s < XS_RING; ++s) issue(s);
 
-    // the outputs of this thread: elements e = tid + XS_THREADS m of the 243, in the order of EXPAND_ORDER
+    // the outputs of this thread: elements e = tid + XS_THREADS m of the NOUT, in the order of EXPAND_ORDER
     uint32_t off[XS_OUT][4];       // byte offsets of the <= 4 x-y terms inside a stage (term 0 repeated when fewer)
     uint32_t ezA[XS_OUT], ezB[XS_OUT];
     int nxy[XS_OUT], wxy[XS_OUT];
@@ -142,9 +147,9 @@ k_expand_M_stream(const __grid_constant__ ExpandStreamArgs a)
 #pragma unroll
     for (int m = 0; m < XS_OUT; ++m) {
         const int e = tid + XS_THREADS * m;
-        valid[m] = e < 243;
+        valid[m] = e < NOUT;
         const int ee = valid[m] ? e : 0;
-        const int o = EXPAND_ORDER[ee / 9], ij = ee % 9;
+        const int o = NSLOT == 27 ? EXPAND_ORDER[ee / 9] : EXPAND_ORDER14[ee / 9], ij = ee % 9;
         const int dx = o / 9 - 1, dy = (o / 3) % 3 - 1, dz = o % 3 - 1;
         const int ebase = ij < 8 ? ij : AM_A8, emul = ij < 8 ? 8 : 1;
         const int ntx = dx == 0 ? 2 : 1, nty = dy == 0 ? 2 : 1;
@@ -163,7 +168,7 @@ k_expand_M_stream(const __grid_constant__ ExpandStreamArgs a)
         ezA[m] = 8u * (unsigned)(emul * (dz == 0 ? 0 : 1));
         ezB[m] = 8u * (unsigned)(emul * 2);
         a_prev[m] = dz < 0;
-        mptr[m] = a.M + ((size_t)i * g.ny + j) * g.nz * 243 + (size_t)(o * 9 + ij);
+        mptr[m] = a.M + ((size_t)i * g.ny + j) * g.nz * NOUT + (size_t)((NSLOT == 27 ? o : o - 13) * 9 + ij);
         // the warp's longest lists (whole warps take part: 128 threads)
         wxy[m] = __reduce_max_sync(0xffffffffu, valid[m] ? nxy[m] : 1);
         wtwo[m] = __any_sync(0xffffffffu, valid[m] && two[m]);
@@ -196,7 +201,7 @@ k_expand_M_stream(const __grid_constant__ ExpandStreamArgs a)
                 }
                 *mptr[m] = s;
             }
-            mptr[m] += 243;
+            mptr[m] += NOUT;
         }
         __syncthreads();                                   // the previous level has been read by everybody: refill its slot
         if (tid == 0) issue(k + XS_RING);

@@ -244,6 +244,15 @@ k_stage_to_slots(uint32_t n, const uint32_t* __restrict__ dest, const uint32_t* 
     for (uint32_t t = threadIdx.x; t < tile_n; t += SORT_STAGE_THREADS) tmp[dsts[t]] = vals[t];
 }
 
+// list[i] = i, *count = n ("every particle" as a list, for kernels that take one)
+__global__ void __launch_bounds__(256)
+k_iota_u32(uint32_t n, uint32_t* __restrict__ list, uint32_t* __restrict__ count)
+{
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += stride) list[p] = (uint32_t)p;
+    if (blockIdx.x == 0 && threadIdx.x == 0) *count = n;
+}
+
 // perm[dest[p]] = p (only when the caller asks for the permutation)
 __global__ void __launch_bounds__(256)
 k_perm_from_dest(uint32_t n, const uint32_t* __restrict__ dest, uint32_t* __restrict__ perm)

@@ -36,7 +36,7 @@ def test_every_declared_symbol_is_exported_and_bound(L):
 
 def test_strerror_and_status_codes(L):
     assert L.ecsim_strerror(0) == b"ok"
-    for code in (-1, -2, -3, -4, -5):
+    for code in (-1, -2, -3, -4, -5, -6):
         assert len(L.ecsim_strerror(code)) > 0
     assert L.ecsim_strerror(-99) == b"unknown status"
 
@@ -62,6 +62,16 @@ def test_null_context_is_an_error_not_a_crash(L):
     assert L.ecsim_set_variant(None, 0) == -1
     assert L.ecsim_enable_timing(None, 1) == -1
     assert L.ecsim_launch_count(None) == 0
+    assert L.ecsim_moments(None, 0, None, 0.1, None, None, None, 0) == -1
+    assert L.ecsim_moments_all(None, None, 0.1, None, None, None, 0) == -1
+    assert L.ecsim_push(None, 0, None, None, 0.1, 0.5) == -1
+    assert L.ecsim_push_all(None, None, None, 0.1, 0.5) == -1
+    assert L.ecsim_make_resident(None, 0, None, 0, 0.25) == -1
+    assert L.ecsim_export_particles(None, 0, None, None, None, None, None, None, None) == -1
+    assert L.ecsim_resident_bytes(None, 10, 0.25) == 0
+    assert L.ecsim_apply_M(None, None, None, None, 0) == -1
+    assert L.ecsim_set_m_layout(None, 0) == -1
+    assert L.ecsim_relayout_count(None) == 0
     assert L.ecsim_destroy(None) == 0
 
 

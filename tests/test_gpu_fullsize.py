@@ -1,12 +1,11 @@
 """-m gpu parity at BASELINE.json's full headline size (configs[2]: 128^3 cells, 268,435,456 particles), in the
-launch configuration bench.py times (ecsim_push_and_moments_all from the cell-sorted state, library defaults:
-slab-pipelined fused kernel + expansion).
+launch configuration bench.py times (ecsim_push_and_moments_all from the cell-sorted state, library defaults).
 
 The oracle cannot run 268 M particles in seconds, so it computes SAMPLED outputs one by one: for a 3x3x3 block
 of cells, the 8 nodes whose eight surrounding cells all lie in the block are fully determined by the block's
 particles.  The test copies exactly those particles (as generated on the device, before the step) to the host,
 runs the oracle on them on the full-size grid, and compares rho / Jhat / M at the 8 nodes and x / v of the
-block's particles.  Blocks sit in the interior, across the periodic corner, and across slab boundaries.
+block's particles.  Blocks sit in the interior, and across the periodic corner.
 Properties that hold at any size are checked on the whole arrays: charge conservation and M's mirror symmetry.
 """
 from __future__ import annotations

@@ -1,6 +1,6 @@
 """-m gpu: randomised parity sweep.  Random small grids (2..9 cells per axis, anisotropic spacing), 1-3 species
 (including a neutral one, q/m = 0), random particle counts (empty species included), random fields, 1-3
-consecutive steps (strays and re-sorts happen), per-species calls or the all-species call, 1-4 slabs.  Every
+consecutive steps (strays and re-sorts happen), per-species calls or the all-species call.  Every
 step is compared with the oracle element by element; the oracle is restarted from the library's particle state
 after each step, so that the 1e-13 bound is a per-step bound (for |beta B| of a few
 hundred the condition number of Eq. 2/6/7 alone exceeds 1e-13/u)."""
@@ -41,7 +41,7 @@ def test_random_case_matches_oracle(seed):
     pcs = [to_cuda(from_numpy(p)) for p in parts]
     ctx = pk.Ecsim(*grid, nsp)
     ctx.set_workspace(max(n + [1]))
-    ctx.set_slabs(int(rng.integers(1, 5)))
+    _ = int(rng.integers(1, 5))          # (a draw the removed slab knob used to take: keeps the seeded cases unchanged)
     ref = []
     for s in range(nsp):
         ctx.load_particles(s, qoms[s], pcs[s], sorted=False)
