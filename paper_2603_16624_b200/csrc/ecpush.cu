@@ -13,6 +13,7 @@
 #include "sort.cuh"
 #include "atomic_path.cuh"
 #include "fused_mma.cuh"
+#include "fused_ws.cuh"
 #include "expand.cuh"
 #include "expand_tma.cuh"
 #include "resident.cuh"
@@ -669,7 +670,7 @@ extern "C" int ecsim_set_resort_fraction(ecsim_ctx* c, double fraction)
 
 extern "C" int ecsim_set_fused_warps(ecsim_ctx* c, int warps)
 {
-    if (!c || (warps != 8 && warps != 12 && warps != 16)) return ECSIM_ERR_INVALID_ARG;
+    if (!c || (warps != 0 && warps != 8 && warps != 12 && warps != 16)) return ECSIM_ERR_INVALID_ARG;
     c->fused_warps = warps;
     return ECSIM_OK;
 }
@@ -734,8 +735,25 @@ static cudaError_t launch_fused(const ecsim_ctx* c, const FusedArgs& fa)
     return cudaGetLastError();
 }
 
+template <int MODE, int LAYOUT>
+static cudaError_t launch_ws(const ecsim_ctx* c, const FusedArgs& fa)
+{
+    cudaError_t e = cudaFuncSetAttribute(k_fused_ws<MODE, LAYOUT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)WS_SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    const size_t cells = (size_t)(fa.c_end - fa.c_begin);
+    size_t grid = (cells + WS_PAIRS - 1) / WS_PAIRS;
+    if (grid > (size_t)c->sm_count) grid = (size_t)c->sm_count;
+    k_fused_ws<MODE, LAYOUT><<<(int)grid, WS_WARPS * 32, WS_SMEM_BYTES, c->stream>>>(fa);
+    return cudaGetLastError();
+}
+
 static cudaError_t launch_fused_any(const ecsim_ctx* c, const FusedArgs& fa, int mode, bool gapped)
 {
+    if (c->fused_warps == 0 && (mode == MODE_FUSED || mode == MODE_MOMENTS)) {
+        if (mode == MODE_FUSED)
+            return gapped ? launch_ws<MODE_FUSED, LAYOUT_GAPPED>(c, fa) : launch_ws<MODE_FUSED, LAYOUT_DENSE>(c, fa);
+        return gapped ? launch_ws<MODE_MOMENTS, LAYOUT_GAPPED>(c, fa) : launch_ws<MODE_MOMENTS, LAYOUT_DENSE>(c, fa);
+    }
     if (mode == MODE_DIAG)
         return gapped ? launch_fused<16, 128, MODE_DIAG, LAYOUT_GAPPED>(c, fa) : launch_fused<16, 128, MODE_DIAG, LAYOUT_DENSE>(c, fa);
     if (mode == MODE_PUSH)
