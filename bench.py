@@ -58,6 +58,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--cpu-sample-planes", type=int, default=8, help="x-planes of cells the oracle sample covers")
+    ap.add_argument("--sustained-steps", type=int, default=-1,
+                    help="consecutive steps WITHOUT restoring the particle state (default: 10; configs[1]: its 1 + 10 protocol; 0 = skip)")
     return ap.parse_args()
 
 
@@ -152,9 +154,11 @@ def workload_name(cfg):
     return f"BASELINE.json configs[{cfg.idx}] {cfg.name}: {cfg.nx}x{cfg.ny}x{cfg.nz} cells, {len(cfg.species)} species"
 
 
-def oracle_sample(cfg, planes, with_e2e_keys=True):
-    """Time the CPU oracle (as it stands: plain C, one thread) on the particles of the first `planes`
-    x-planes of cells of the workload, on the full-size grid.  Returns (particles/s, n, seconds, cores)."""
+def oracle_sample(cfg, planes, all_cores=True):
+    """Time the CPU oracle (oracle/ecsim_oracle.c as it stands: plain C, gcc -O2 -ffp-contract=off) on the particles of
+    the first `planes` x-planes of cells of the workload, on the full-size grid.  all_cores: through
+    oracle.step_planes, which calls the same per-particle loop per x-plane of cells, even planes in parallel, then odd
+    planes (no arithmetic of its own).  Returns (particles/s, n, seconds, threads used)."""
     import numpy as np
     import oracle
     import workloads as wl
@@ -165,13 +169,20 @@ def oracle_sample(cfg, planes, with_e2e_keys=True):
     En, Bn = E.numpy(), B.numpy()
     parts = [to_numpy(wl.gen_species(cfg, s, cells=cells)) for s in range(len(cfg.species))]
     n = sum(p["x"].shape[0] for p in parts)
+    _, start = wl.cell_layout(cfg)
+    plane_start = start.numpy()[::cfg.ny * cfg.nz].copy()
+    plane_start[planes:] = plane_start[planes]           # planes beyond the sample hold no particles
     mom = oracle.Moments(cfg.nodes, with_abs=False)      # calloc-backed: only touched pages are committed
     oracle.lib()
+    threads = oracle.threads() if all_cores else 1
     t0 = time.perf_counter()
     for s, sp in enumerate(cfg.species):
-        oracle.step(grid_of(cfg), sp.qom, cfg.dt, parts[s], En, Bn, mom)
+        if all_cores:
+            oracle.step_planes(grid_of(cfg), sp.qom, cfg.dt, parts[s], plane_start, En, Bn, mom)
+        else:
+            oracle.step(grid_of(cfg), sp.qom, cfg.dt, parts[s], En, Bn, mom)
     dt = time.perf_counter() - t0
-    return n / dt, n, dt, 1
+    return n / dt, n, dt, threads
 
 
 def run_reference(args):
@@ -185,6 +196,7 @@ def run_reference(args):
     for _ in range(max(1, args.steps)):
         r, n, dt, cores = oracle_sample(cfg, args.cpu_sample_planes)
         rates.append(r); secs.append(dt)
+    cores = rates and cores or 1
     value = n * len(secs) / sum(secs)
     sample = (f"particles of the first {min(args.cpu_sample_planes, cfg.nx)} x-planes of cells "
               f"({n} particles, all species) on the full {cfg.nx}x{cfg.ny}x{cfg.nz} grid, one oracle step per bench step")
@@ -193,8 +205,9 @@ def run_reference(args):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sum(secs) / len(secs),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(cfg), "note": "CPU oracle (oracle/ecsim_oracle.c, gcc -O2 -ffp-contract=off), "
-                   "host cores of this box; ms_per_step is per sample, not per full workload"},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+                   "all host cores of this box (x-planes of cells in two colours); ms_per_step is per sample, not per full workload"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "host_cores": os.cpu_count(), "kind": "oracle",
+                         "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -248,13 +261,17 @@ def run_product(args):
     M = torch.empty(cfg.nodes, 27, 3, 3, dtype=torch.float64, device=dev)
     sorted_input = not cfg.shuffled
 
-    def restore():
+    def restore_arrays():
         for s in range(nsp):
             for k in ("x", "y", "z", "u", "v", "w") + (("q",) if cfg.shuffled else ()):
                 work[s][k].copy_(pristine[s][k])
             ctx.load_particles(s, cfg.species[s].qom, work[s], sorted=sorted_input)
-            if sorted_input:
-                ctx.build_segments(s)        # set-up of the sorted state, not part of the step
+
+    def restore():
+        restore_arrays()
+        if sorted_input:
+            for s in range(nsp):
+                ctx.build_segments(s)        # set-up of the sorted state, not part of the step ("step_with_segments_ms" has it inside)
 
     def one_step():
         ctx.push_and_moments_all(E, B, cfg.dt, cfg.theta, rho, J, M, accumulate=pk.ACC_NONE)
@@ -323,19 +340,31 @@ def run_product(args):
         "clocks": clocks,
     }
 
+    # ---- what a time loop sees: the step WITH the segment-table build, and consecutive steps ----
+    line["step_with_segments_ms"] = measure_with_segments(args, cfg, ctx, restore_arrays, one_step, world)
+    n_sus = args.sustained_steps if args.sustained_steps >= 0 else (cfg.steps if cfg.steps > 1 else 10)
+    if n_sus > 0:
+        line["sustained"] = measure_sustained(args, cfg, ctx, restore_arrays, work, E, B, rho, J, M, n_sus, n_total, world)
+    else:
+        line["sustained"] = None
+
     # ---- end to end through the host-buffer entry point (rank-local, pinned host memory) ----
+    ctx.close()
+    del work, M, rho, J
+    torch.cuda.empty_cache()
     if not args.no_e2e:
-        line["e2e"] = run_e2e(args, cfg, ctx, pristine, E, B, world)
+        line["e2e"] = run_e2e(args, cfg, None, pristine, E, B, world)
     else:
         line["e2e"] = None
-    ctx.close()
-    del work, pristine, M
+    del pristine
     torch.cuda.empty_cache()
 
     if rank == 0 and not args.no_cpu_baseline and world == 1:
         v, n, dt, cores = oracle_sample(cfg, args.cpu_sample_planes)
+        v1, n1, dt1, _ = oracle_sample(cfg, max(1, args.cpu_sample_planes // 8), all_cores=False)
         line["cpu_baseline"] = {
-            "value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "value": v, "unit": UNIT, "cores": cores, "host_cores": os.cpu_count(), "kind": "oracle",
+            "single_thread_value": v1,
             "sample": f"particles of the first {min(args.cpu_sample_planes, cfg.nx)} x-planes of cells ({n} particles, "
                       f"all species) on the full grid; {dt:.1f} s of CPU work"}
     else:
@@ -344,6 +373,66 @@ def run_product(args):
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+
+
+def _median(v):
+    return statistics.median(v) if v else None
+
+
+def measure_with_segments(args, cfg, ctx, restore_arrays, one_step, world):
+    """The headline step with the per-species segment tables (histogram + scan of cell-sorted arrays) built INSIDE the
+    timed region: what the first step after a load costs."""
+    import torch
+    ms = []
+    for _ in range(3):
+        restore_arrays()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); one_step(); e1.record()
+        torch.cuda.synchronize()
+        ms.append(e0.elapsed_time(e1))
+    return max_over_ranks([_median(ms)], world)[0]
+
+
+def measure_sustained(args, cfg, ctx, restore_arrays, work, E, B, rho, J, M, n_steps, n_total, world):
+    """n_steps CONSECUTIVE steps, fields fixed, particle state never restored (configs[1]'s protocol; 10 steps of the
+    headline workload by default): every stray, re-sort and fresh layout is inside the timed steps.
+      dense:    the caller's arrays pushed in place (ecsim_push_and_moments_all): leavers become strays, re-sorts by rent-or-buy
+      resident: library-managed gapped double buffers (ecsim_make_resident): the sort-preserving push, no strays."""
+    import torch
+    import paper_2603_16624_b200 as pk
+    nsp = len(cfg.species)
+    out = {}
+    for kind in ("dense", "resident"):
+        restore_arrays()
+        if kind == "resident":
+            free, _ = torch.cuda.mem_get_info()
+            need = sum(ctx.resident_bytes(int(work[s]["x"].numel()), 0.5) for s in range(nsp))
+            if need > free - (2 << 30):
+                out[kind] = {"skipped": f"needs {need / 1e9:.1f} GB of device memory, {free / 1e9:.1f} GB free"}
+                continue
+            for s in range(nsp):
+                ctx.make_resident(s, 0.5)
+        torch.cuda.synchronize()
+        r0, l0 = ctx.resort_count(), ctx.relayout_count()
+        ms, strays, leavers = [], [], []
+        for _ in range(n_steps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            ctx.push_and_moments_all(E, B, cfg.dt, cfg.theta, rho, J, M, accumulate=pk.ACC_NONE)
+            e1.record()
+            torch.cuda.synchronize()
+            ms.append(e0.elapsed_time(e1))
+            strays.append(ctx.stray_count())
+            leavers.append(ctx.leaver_count())
+        tot = max_over_ranks([sum(ms)], world)[0]
+        out[kind] = {"steps": n_steps, "ms_per_step": tot / n_steps, "ms_first": ms[0], "ms_each": [round(v, 3) for v in ms],
+                     "ms_median_after_first": _median(ms[1:]) if len(ms) > 1 else None,
+                     "particles_per_s": world * n_total * n_steps / (tot * 1e-3),
+                     "north_star_frac": n_total * n_steps / (tot * 1e-3) / NORTH_STAR_ROOFLINE_PPS,
+                     "strays_per_step": strays, "leavers_per_step": leavers,
+                     "resorts": ctx.resort_count() - r0, "relayouts": ctx.relayout_count() - l0}
+    return out
 
 
 def run_e2e(args, cfg, ctx_unused, pristine, E, B, world):

@@ -152,12 +152,13 @@ int ecsim_push_all(ecsim_ctx *ctx, const double *E_theta, const double *B, doubl
  * ecsim_make_resident bins a loaded species and copies it into two library-managed buffers inside dev_buf (device
  * memory lent by the caller until ecsim_destroy / the next ecsim_load_particles of that species; 256-byte aligned,
  * ecsim_resident_bytes(ctx, n, slack) large).  Each cell owns a segment of slots in both buffers: its particles plus
- * max(8, slack * particles) spare slots.  From then on every push of that species (ecsim_push, ecsim_push_and_moments,
+ * max(8, slack * max(particles, mean particles per cell)) spare slots.  From then on every push of that species (ecsim_push, ecsim_push_and_moments,
  * *_all) reads one buffer and writes the other: particles that stay in their cell are written, compacted, to the front
  * of the cell's segment, a particle that moves to another cell is written straight to the back of THAT cell's segment.
  * Every step therefore starts from cell-sorted particles: no strays, no re-sort.  A particle whose new cell has no free
- * slot goes to an overflow list (n/8 entries); the next call then lays the species out afresh (counted by
- * ecsim_relayout_count).  The arrays given to ecsim_load_particles are not referenced after ecsim_make_resident returns
+ * slot goes to an overflow list (n/8 entries) and is handled, one warp per particle, by every later pass until a slot
+ * is free; when the list has cost more than a fresh layout (ecsim_set_resort_fraction, as for the re-sort of a dense
+ * species) the species is laid out afresh (counted by ecsim_relayout_count).  The arrays given to ecsim_load_particles are not referenced after ecsim_make_resident returns
  * and are NOT updated by pushes: read the species back with ecsim_export_particles (device arrays of n doubles each;
  * cell-major order; also works, as a plain copy, for a species that is not resident).
  * ecsim_make_resident synchronises the stream once (it checks the data-dependent slot count against the buffer);
@@ -167,6 +168,16 @@ int ecsim_make_resident(ecsim_ctx *ctx, int species, void *dev_buf, size_t bytes
 int ecsim_export_particles(ecsim_ctx *ctx, int species, double *x, double *y, double *z, double *u, double *v,
                            double *w, double *q);
 int64_t ecsim_relayout_count(const ecsim_ctx *ctx);
+
+/* Reduced dimensionality (L123: "fixPosition ... is only called if the simulation is one or two-dimensional and set the
+ * particle position along the same line or on the same plane.  This step is necessary to ensure the correctness of the
+ * mass matrix calculations").  axis_mask: bit 0 x, bit 1 y, bit 2 z; from this call on every push (all variants, all
+ * layouts) overwrites the masked coordinates of the pushed position with px / py / pz (each in [0, L)) before the
+ * periodic wrap; velocities keep all three components.  Species already loaded are pinned by the call (and re-binned
+ * before their next step); ecsim_load_particles pins on load while a mask is set (the one case where a load enqueues
+ * device work).  A 2-D run in the x-y plane: any nz >= 2, axis_mask = 4, pz = a node plane k0*dz: every z weight is
+ * (1, 0), all moments land on node plane k0.  axis_mask = 0 switches the pinning off. */
+int ecsim_set_fixed_axes(ecsim_ctx *ctx, int axis_mask, double px, double py, double pz);
 
 /* Diagnostic moments of one species, the quantities ECsim writes with its I/O (L121 "plasma density, current, pressure,
  * and heat flux"; L147 computeCharge / computeCurrent: "The diagnostic charge current differs from J-hat, as it excludes

@@ -33,6 +33,14 @@ def lib():
             [ctypes.c_int] * 3 + [ctypes.c_double] * 3 + [ctypes.c_int64] + [_D] * 3 + [_I32, _I32])
         _lib.ecsim_oracle_apply_M.restype = ctypes.c_int
         _lib.ecsim_oracle_apply_M.argtypes = [ctypes.c_int] * 3 + [_D] * 3
+        _lib.ecsim_oracle_fix_position.restype = ctypes.c_int
+        _lib.ecsim_oracle_fix_position.argtypes = [ctypes.c_int64] + [_D] * 3 + [ctypes.c_int] + [ctypes.c_double] * 3
+        _lib.ecsim_oracle_threads.restype = ctypes.c_int
+        _lib.ecsim_oracle_threads.argtypes = []
+        _lib.ecsim_oracle_step_planes.restype = ctypes.c_int
+        _lib.ecsim_oracle_step_planes.argtypes = (
+            [ctypes.c_int] * 3 + [ctypes.c_double] * 3 + [ctypes.POINTER(ctypes.c_int64), ctypes.c_double, ctypes.c_double]
+            + [_D] * 6 + [_D] * 3 + [_D] * 3 + [ctypes.c_int])
         _lib.ecsim_oracle_diagnostics.restype = ctypes.c_int
         _lib.ecsim_oracle_diagnostics.argtypes = ([ctypes.c_int] * 3 + [ctypes.c_double] * 3 + [ctypes.c_int64]
                                                   + [_D] * 7 + [_D] * 4 + [_D] * 4)
@@ -118,4 +126,30 @@ def diagnostics(grid, part: dict, diag: Diagnostics):
         nx, ny, nz, dx, dy, dz, n, _p(part["x"]), _p(part["y"]), _p(part["z"]), _p(part["u"]), _p(part["v"]),
         _p(part["w"]), _p(part["q"]), _p(diag.rho), _p(diag.J), _p(diag.P), _p(diag.Q),
         _p(diag.rho_abs), _p(diag.J_abs), _p(diag.P_abs), _p(diag.Q_abs))
+    assert rc == 0
+
+
+def threads() -> int:
+    """Threads the timing variant `step_planes` will use (OpenMP max threads)."""
+    return int(lib().ecsim_oracle_threads())
+
+
+def step_planes(grid, qom: float, dt: float, part: dict, plane_start: np.ndarray, E: np.ndarray, B: np.ndarray,
+                mom: Moments, push: bool = True):
+    """TIMING VARIANT on all host cores: `step` called per x-plane of cells, even planes in parallel, then odd planes
+    (no arithmetic of its own).  `part` must be ordered by x-plane of cells, plane i = [plane_start[i], plane_start[i+1])."""
+    nx, ny, nz, dx, dy, dz = grid
+    ps = np.ascontiguousarray(plane_start, dtype=np.int64)
+    assert ps.shape[0] == nx + 1
+    rc = lib().ecsim_oracle_step_planes(
+        nx, ny, nz, dx, dy, dz, ps.ctypes.data_as(ctypes.POINTER(ctypes.c_int64)), qom, dt,
+        _p(part["x"]), _p(part["y"]), _p(part["z"]), _p(part["u"]), _p(part["v"]), _p(part["w"]),
+        _p(part["q"]), _p(E), _p(B), _p(mom.rho), _p(mom.J), _p(mom.M), 1 if push else 0)
+    assert rc == 0, "particles are not ordered by x-plane of cells"
+
+
+def fix_position(part: dict, axis_mask: int, px: float = 0.0, py: float = 0.0, pz: float = 0.0):
+    """fixPosition (reading R25): pin the coordinates of the masked axes in place."""
+    rc = lib().ecsim_oracle_fix_position(part["x"].shape[0], _p(part["x"]), _p(part["y"]), _p(part["z"]), axis_mask,
+                                         px, py, pz)
     assert rc == 0

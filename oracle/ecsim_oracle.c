@@ -287,3 +287,69 @@ int ecsim_oracle_diagnostics(int nx, int ny, int nz, double dx, double dy, doubl
     }
     return 0;
 }
+
+/*
+ * TIMING VARIANT of ecsim_oracle_step on all host cores (SURVEY §8(d) "oracle_omp"; reported beside the GPU number,
+ * never the parity reference).  No arithmetic of its own: it calls ecsim_oracle_step on the particles of one x-plane
+ * of cells at a time.  The particles must be ordered by x-plane of cells: plane i = [plane_start[i], plane_start[i+1]).
+ * A plane of cells deposits only on the node planes i and i+1, so planes of the same parity never touch the same node
+ * (nx even, or nx odd and the last plane taken alone): even planes run in parallel, then odd planes.  Per-node summation
+ * order differs from the sequential loop, results agree to rounding (tests: <= 1e-12 of the |addend| sums).
+ * Returns -1 if a particle is not in the plane its range claims.
+ */
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+int ecsim_oracle_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+int ecsim_oracle_step_planes(int nx, int ny, int nz, double dx, double dy, double dz,
+                             const int64_t *plane_start /* [nx+1] */, double qom, double dt,
+                             double *x, double *y, double *z, double *u, double *v, double *w,
+                             const double *q, const double *E, const double *B,
+                             double *rho, double *J, double *M, int do_push)
+{
+    const double rdx = 1.0 / dx;
+    int bad = 0;
+    for (int i = 0; i < nx && !bad; ++i)
+        for (int64_t p = plane_start[i]; p < plane_start[i + 1]; ++p)
+            if (lower_node(x[p] * rdx, nx) != i) { bad = 1; break; }
+    if (bad) return -1;
+    const int last_alone = (nx % 2) != 0;        /* odd nx: plane nx-1 and plane 0 are both even and share node plane 0 */
+    for (int colour = 0; colour < 2; ++colour) {
+#pragma omp parallel for schedule(dynamic, 1)
+        for (int i = colour; i < nx - last_alone; i += 2) {
+            const int64_t o = plane_start[i], n = plane_start[i + 1] - o;
+            ecsim_oracle_step(nx, ny, nz, dx, dy, dz, n, qom, dt, x + o, y + o, z + o, u + o, v + o, w + o, q + o, E, B,
+                              rho, J, M, NULL, NULL, NULL, NULL, do_push);
+        }
+    }
+    if (last_alone) {
+        const int64_t o = plane_start[nx - 1], n = plane_start[nx] - o;
+        ecsim_oracle_step(nx, ny, nz, dx, dy, dz, n, qom, dt, x + o, y + o, z + o, u + o, v + o, w + o, q + o, E, B,
+                          rho, J, M, NULL, NULL, NULL, NULL, do_push);
+    }
+    return 0;
+}
+
+/*
+ * fixPosition: "only called if the simulation is one or two-dimensional and set the particle position
+ * along the same line or on the same plane.  This step is necessary to ensure the correctness of the mass matrix
+ * calculations in case of reduced simulation dimensions."  Reading R25: after updatePosition the coordinates
+ * of the inactive axes (axis_mask bit 0 x, 1 y, 2 z) are overwritten with fixed values; velocities keep three components.
+ */
+int ecsim_oracle_fix_position(int64_t n, double *x, double *y, double *z, int axis_mask, double px, double py, double pz)
+{
+    for (int64_t p = 0; p < n; ++p) {
+        if (axis_mask & 1) x[p] = px;
+        if (axis_mask & 2) y[p] = py;
+        if (axis_mask & 4) z[p] = pz;
+    }
+    return 0;
+}

@@ -64,6 +64,7 @@ _PROTOS = {
     "ecsim_relayout_count": (_c.c_int64, [_P]),
     "ecsim_apply_M": (_c.c_int, [_P, _P, _P, _P, _c.c_int]),
     "ecsim_diagnostics": (_c.c_int, [_P, _c.c_int, _P, _P, _P, _P]),
+    "ecsim_set_fixed_axes": (_c.c_int, [_P, _c.c_int, _c.c_double, _c.c_double, _c.c_double]),
     "ecsim_host_step_workspace_bytes": (_c.c_size_t, [_P, _c.c_int64]),
     "ecsim_push_and_moments_host": (_c.c_int, [_P, _c.c_int64, _c.c_double, _c.c_int] + [_P] * 9 +
                                     [_c.c_double, _c.c_double, _P, _P, _P, _c.c_int]),
@@ -243,6 +244,9 @@ class Ecsim:
 
     def relayout_count(self) -> int:
         return int(self.L.ecsim_relayout_count(self.h))
+
+    def set_fixed_axes(self, axis_mask: int, px: float = 0.0, py: float = 0.0, pz: float = 0.0):
+        _check(self.L.ecsim_set_fixed_axes(self.h, axis_mask, px, py, pz), "ecsim_set_fixed_axes")
 
     def diagnostics(self, species: int, rho, J, P, Q):
         f64 = self.torch.float64

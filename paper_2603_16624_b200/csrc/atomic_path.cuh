@@ -115,9 +115,9 @@ k_push_moments_atomic(AtomicArgs a)
         const double vby = al[3] * tx + al[4] * ty + al[5] * tz;
         const double vbz = al[6] * tx + al[7] * ty + al[8] * tz;
         const double un = 2.0 * vbx - vx, vn = 2.0 * vby - vy, wn = 2.0 * vbz - vz;
-        const double xn = wrap_periodic(x + a.dt * un, g.Lx);
-        const double yn = wrap_periodic(y + a.dt * vn, g.Ly);
-        const double zn = wrap_periodic(z + a.dt * wn, g.Lz);
+        double xn = x + a.dt * un, yn = y + a.dt * vn, zn = z + a.dt * wn;
+        pin_axes(g, xn, yn, zn);
+        xn = wrap_periodic(xn, g.Lx); yn = wrap_periodic(yn, g.Ly); zn = wrap_periodic(zn, g.Lz);
         a.u[p] = un; a.v[p] = vn; a.w[p] = wn;
         a.x[p] = xn; a.y[p] = yn; a.z[p] = zn;
         if (USE_LIST) {
@@ -255,9 +255,11 @@ k_push_strays_bulk(StrayArgs a, int am_per_cell, int am_a8)
             const double vn = 2.0 * (al[3] * tx + al[4] * ty + al[5] * tz) - vy;
             const double wn = 2.0 * (al[6] * tx + al[7] * ty + al[8] * tz) - vz;
             a.u[p] = un; a.v[p] = vn; a.w[p] = wn;
-            a.x[p] = wrap_periodic(x + a.dt * un, g.Lx);
-            a.y[p] = wrap_periodic(y + a.dt * vn, g.Ly);
-            a.z[p] = wrap_periodic(z + a.dt * wn, g.Lz);
+            double xn = x + a.dt * un, yn = y + a.dt * vn, zn = z + a.dt * wn;
+            pin_axes(g, xn, yn, zn);
+            a.x[p] = wrap_periodic(xn, g.Lx);
+            a.y[p] = wrap_periodic(yn, g.Ly);
+            a.z[p] = wrap_periodic(zn, g.Lz);
             my_leavers += 1;   // a stray stays outside the segment it is stored in
         }
         if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the staging block may be rewritten
@@ -271,8 +273,9 @@ k_push_strays_bulk(StrayArgs a, int am_per_cell, int am_a8)
 // arrays, after the expansion wrote them.
 struct DiagStrayArgs {
     Geom g;
-    const uint32_t* list;
+    const uint32_t* list;        // indices, or null: entries 0..count-1 themselves
     const uint32_t* list_count;
+    uint32_t count_cap;          // the count is clamped to this
     const double *x, *y, *z, *u, *v, *w, *q;
     double *rho, *J, *P, *Q;
 };
@@ -281,10 +284,10 @@ __global__ void __launch_bounds__(128)
 k_diag_strays(DiagStrayArgs a)
 {
     const Geom& g = a.g;
-    const size_t count = (size_t)*a.list_count;
+    const size_t count = (size_t)min(*a.list_count, a.count_cap);
     const size_t stride = (size_t)gridDim.x * blockDim.x;
     for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < count; t += stride) {
-        const size_t p = a.list[t];
+        const size_t p = a.list ? a.list[t] : t;
         const double sx = a.x[p] * g.rdx, sy = a.y[p] * g.rdy, sz = a.z[p] * g.rdz;
         const int i0 = lower_node(sx, g.nx), j0 = lower_node(sy, g.ny), k0 = lower_node(sz, g.nz);
         const int i1 = (i0 + 1 == g.nx) ? 0 : i0 + 1, j1 = (j0 + 1 == g.ny) ? 0 : j0 + 1, k1 = (k0 + 1 == g.nz) ? 0 : k0 + 1;

@@ -15,7 +15,21 @@ struct Geom {
     double Lx, Ly, Lz;      // box lengths n*d
     double invV;            // 1/(dx dy dz): V_N is the same for every node of a periodic grid (L49)
     long long nodes;
+    // reduced dimensionality (fixPosition, L123): coordinates of the axes in fix_mask (bit 0 x, 1 y, 2 z) are pinned
+    // to fix_pos[axis] by every push, so that all particles stay on one line / plane of the grid
+    int fix_mask;
+    double fix_pos[3];
 };
+
+// fixPosition (L123): "set the particle position along the same line or on the same plane" after updatePosition.
+__device__ __forceinline__ void pin_axes(const Geom& g, double& x, double& y, double& z)
+{
+    if (g.fix_mask) {
+        if (g.fix_mask & 1) x = g.fix_pos[0];
+        if (g.fix_mask & 2) y = g.fix_pos[1];
+        if (g.fix_mask & 4) z = g.fix_pos[2];
+    }
+}
 
 // A particle's lower node N- per axis (L131): floor(x/dx) clamped into the grid.
 __device__ __forceinline__ int lower_node(double s, int n)

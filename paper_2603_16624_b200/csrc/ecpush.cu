@@ -17,6 +17,7 @@
 #include "expand.cuh"
 #include "expand_tma.cuh"
 #include "resident.cuh"
+#include "homeless.cuh"
 #include "apply_m.cuh"
 #include "probe.cuh"
 
@@ -49,9 +50,10 @@ struct Resident {
     uint32_t* F[2] = {};            // [cells] front runs
     uint32_t* R[2] = {};            // [cells] back runs (arrivals of the last push)
     int cur = 0;                    // buffer that holds the species now
-    double* ovf = nullptr;          // [7][ovf_cap] overflow list of the last push
+    double* ovf[2] = {};            // two overflow lists [7][ovf_cap]: particles without a slot ("homeless")
     uint32_t ovf_cap = 0;
-    uint32_t* ovf_count = nullptr;  // device counter
+    uint32_t* ovf_count[2] = {};    // device counters
+    int ovf_cur = 0;                // list that holds the homeless particles now (a push reads it and fills the other)
 };
 
 struct SpeciesHost {
@@ -210,6 +212,8 @@ extern "C" int ecsim_init_grid(ecsim_ctx** ctx, int nx, int ny, int nz, double d
     g.Lx = nx * dx; g.Ly = ny * dy; g.Lz = nz * dz;
     g.invV = 1.0 / (dx * dy * dz);
     g.nodes = (long long)nx * ny * nz;
+    g.fix_mask = 0;
+    g.fix_pos[0] = g.fix_pos[1] = g.fix_pos[2] = 0.0;
     c->n_species = n_species;
     c->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
     c->sm_count = prop.multiProcessorCount;
@@ -309,6 +313,55 @@ extern "C" int ecsim_load_particles(ecsim_ctx* c, int s, int64_t n, double q_ove
     sp.stray_debt = 0.0;
     sp.leavers_pending = false;
     sp.res.on = false;              // a fresh load is a borrowed (dense) species again
+    if (c->g.fix_mask && n > 0) {
+        // reduced dimensionality: the species starts on the line / plane (the one load that enqueues device work)
+        k_fix_position<<<grid_for(c, (size_t)n, 256, 16), 256, 0, c->stream>>>(c->g, (size_t)n, x, y, z);
+        CK_LAUNCH();
+        c->launches++;
+    }
+    return ECSIM_OK;
+}
+
+static int resident_settle(ecsim_ctx* c, int s);
+static int resident_relayout(ecsim_ctx* c, int s);
+
+// Reduced dimensionality (L123 fixPosition): from now on every push pins the coordinates of the axes in axis_mask
+// (bit 0 x, 1 y, 2 z) to the given values; species already loaded are pinned now.
+extern "C" int ecsim_set_fixed_axes(ecsim_ctx* c, int axis_mask, double px, double py, double pz)
+{
+    if (!c || axis_mask < 0 || axis_mask > 7) return ECSIM_ERR_INVALID_ARG;
+    const double pos[3] = {px, py, pz};
+    const double L[3] = {c->g.Lx, c->g.Ly, c->g.Lz};
+    for (int a = 0; a < 3; ++a)
+        if ((axis_mask >> a) & 1)
+            if (!(pos[a] >= 0.0 && pos[a] < L[a])) return ECSIM_ERR_INVALID_ARG;
+    c->g.fix_mask = axis_mask;
+    for (int a = 0; a < 3; ++a) c->g.fix_pos[a] = pos[a];
+    if (!axis_mask) return ECSIM_OK;
+    for (int s = 0; s < c->n_species; ++s) {
+        SpeciesHost& sp = c->sp[s];
+        if (!sp.loaded || sp.n == 0) continue;
+        if (sp.res.on) {
+            // every slot of both buffers (unused slots hold nothing that matters); cells along a pinned axis do not change
+            int rc = resident_settle(c, s);
+            if (rc) return rc;
+            for (int b = 0; b < 2; ++b) {
+                k_fix_position<<<c->sm_count * 8, 256, 0, c->stream>>>(c->g, (size_t)sp.res.cap_bound, sp.res.buf[b][0],
+                                                                         sp.res.buf[b][1], sp.res.buf[b][2]);
+                CK_LAUNCH();
+                c->launches++;
+            }
+            // the pinned particles may now sit in other cells than their segments say: lay the species out afresh
+            rc = resident_relayout(c, s);
+            if (rc) return rc;
+        } else {
+            k_fix_position<<<grid_for(c, (size_t)sp.n, 256, 16), 256, 0, c->stream>>>(c->g, (size_t)sp.n, sp.x, sp.y, sp.z);
+            CK_LAUNCH();
+            c->launches++;
+            sp.state = ST_UNSORTED;
+            sp.nearly_sorted = false;
+        }
+    }
     return ECSIM_OK;
 }
 
@@ -469,8 +522,8 @@ extern "C" int ecsim_cell_index(ecsim_ctx* c, int s, int32_t* cell_out)
 static size_t resident_tables_bytes(const ecsim_ctx* c, uint32_t ovf_cap)
 {
     const size_t cells = (size_t)c->g.nodes;
-    return align_up(sizeof(uint32_t) * (cells + 1), 256) + 4 * align_up(sizeof(uint32_t) * cells, 256) + 256 +
-           align_up(sizeof(double) * 7 * (size_t)ovf_cap, 256);
+    return align_up(sizeof(uint32_t) * (cells + 1), 256) + 4 * align_up(sizeof(uint32_t) * cells, 256) + 2 * 256 +
+           2 * align_up(sizeof(double) * 7 * (size_t)ovf_cap, 256);
 }
 
 static uint32_t resident_ovf_cap(int64_t n)
@@ -486,8 +539,8 @@ extern "C" size_t ecsim_resident_bytes(const ecsim_ctx* c, int64_t n, double sla
 {
     if (!c || n < 0 || !(slack >= 0.0) || slack > 4.0) return 0;
     const size_t cells = (size_t)c->g.nodes;
-    // slots: n + ceil(slack n_c) per cell + the minimum slack and the rounding to 4 per cell
-    const size_t slots = (size_t)n + (size_t)ceil(slack * (double)n) + (RESIDENT_MIN_SLACK + 4) * cells + 64;
+    // slots: n + ceil(slack max(n_c, mean)) per cell (<= slack n + slack n) + the minimum slack and the rounding to 4 per cell
+    const size_t slots = (size_t)n + 2 * (size_t)ceil(slack * (double)n) + (RESIDENT_MIN_SLACK + 4) * cells + 64;
     return resident_tables_bytes(c, resident_ovf_cap(n)) + 14 * align_up(sizeof(double) * slots, 256);
 }
 
@@ -504,7 +557,7 @@ static int resident_layout_from_dense(ecsim_ctx* c, int s, const double* const s
     if (rc) return rc;
     const int cgrid = (int)((cells + 255) / 256);
     uint32_t* cap = r.R[dst_buf];              // scratch until the runs are written
-    k_gapped_caps<<<cgrid, 256, 0, c->stream>>>(cells, w.count, r.slack, RESIDENT_MIN_SLACK, cap);
+    k_gapped_caps<<<cgrid, 256, 0, c->stream>>>(cells, w.count, r.slack, RESIDENT_MIN_SLACK, (double)n / (double)cells, cap);
     CK_LAUNCH();
     c->launches++;
     rc = scan_u32(c, cap, r.seg, cells);
@@ -547,7 +600,7 @@ static int resident_export(ecsim_ctx* c, int s, double* const dst[7], bool with_
     CK_LAUNCH();
     c->launches++;
     if (with_overflow) {
-        k_append_overflow<<<c->sm_count, 256, 0, c->stream>>>(r.ovf_count, r.ovf_cap, r.ovf, start + cells, out);
+        k_append_overflow<<<c->sm_count, 256, 0, c->stream>>>(r.ovf_count[r.ovf_cur], r.ovf_cap, r.ovf[r.ovf_cur], start + cells, out);
         CK_LAUNCH();
         c->launches++;
     }
@@ -565,7 +618,10 @@ static int resident_relayout(ecsim_ctx* c, int s)
     for (int k = 0; k < 7; ++k) src[k] = r.buf[other][k];
     rc = resident_layout_from_dense(c, s, src, r.cur);
     if (rc) return rc;
-    CK(cudaMemsetAsync(r.ovf_count, 0, sizeof(uint32_t), c->stream));
+    CK(cudaMemsetAsync(r.ovf_count[0], 0, sizeof(uint32_t), c->stream));
+    CK(cudaMemsetAsync(r.ovf_count[1], 0, sizeof(uint32_t), c->stream));
+    c->sp[s].stray_debt = 0.0;
+    c->h_ovf[s] = 0;
     c->relayouts++;
     return ECSIM_OK;
 }
@@ -589,8 +645,10 @@ extern "C" int ecsim_make_resident(ecsim_ctx* c, int s, void* dev_buf, size_t by
     r.seg = k.take<uint32_t>(cells + 1);
     r.F[0] = k.take<uint32_t>(cells); r.F[1] = k.take<uint32_t>(cells);
     r.R[0] = k.take<uint32_t>(cells); r.R[1] = k.take<uint32_t>(cells);
-    r.ovf_count = k.take<uint32_t>(1);
-    r.ovf = k.take<double>(7 * (size_t)r.ovf_cap);
+    r.ovf_count[0] = k.take<uint32_t>(1);
+    r.ovf_count[1] = k.take<uint32_t>(1);
+    r.ovf[0] = k.take<double>(7 * (size_t)r.ovf_cap);
+    r.ovf[1] = k.take<double>(7 * (size_t)r.ovf_cap);
     const size_t per_array = ((bytes - k.off) / 14) & ~(size_t)255;
     size_t slots = per_array / sizeof(double);
     if (slots > 0xfffffff0u) slots = 0xfffffff0u;
@@ -606,7 +664,8 @@ extern "C" int ecsim_make_resident(ecsim_ctx* c, int s, void* dev_buf, size_t by
     const double* src[7] = {sp.x, sp.y, sp.z, sp.u, sp.v, sp.w, sp.q};
     rc = resident_layout_from_dense(c, s, src, 0);
     if (rc) return rc;
-    CK(cudaMemsetAsync(sp.res.ovf_count, 0, sizeof(uint32_t), c->stream));
+    CK(cudaMemsetAsync(sp.res.ovf_count[0], 0, sizeof(uint32_t), c->stream));
+    CK(cudaMemsetAsync(sp.res.ovf_count[1], 0, sizeof(uint32_t), c->stream));
     sp.res.on = true;
     sp.state = ST_SEGMENTED;
     sp.leavers_pending = false;
@@ -615,8 +674,9 @@ extern "C" int ecsim_make_resident(ecsim_ctx* c, int s, void* dev_buf, size_t by
     return ECSIM_OK;
 }
 
-// Before a call touches a resident species: the overflow counter of its last push (host-visible once that push has
-// finished) decides whether the species must be laid out afresh.
+// Before a call touches a resident species: the size of its overflow list after its last push (host-visible once that
+// push has finished).  Homeless particles cost a stray-kernel warp each per step (homeless.cuh); a fresh layout costs
+// about as much as a re-sort: rent or buy, with the same knob as the dense layout (ecsim_set_resort_fraction).
 static int resident_settle(ecsim_ctx* c, int s)
 {
     SpeciesHost& sp = c->sp[s];
@@ -624,10 +684,8 @@ static int resident_settle(ecsim_ctx* c, int s)
     CK(cudaEventSynchronize(sp.leavers_event));
     sp.leavers_pending = false;
     if (c->h_ovf[s] > sp.res.ovf_cap) return ECSIM_ERR_OVERFLOW;
-    if (c->h_ovf[s] > 0) {
-        c->h_ovf[s] = 0;
-        return resident_relayout(c, s);
-    }
+    sp.stray_debt += (double)c->h_ovf[s];
+    if (c->h_ovf[s] > 0 && sp.stray_debt > 0.25 * c->resort_fraction * (double)sp.n) return resident_relayout(c, s);   // (a homeless particle costs ~4x a stray)
     return ECSIM_OK;
 }
 
@@ -648,7 +706,7 @@ extern "C" int ecsim_export_particles(ecsim_ctx* c, int s, double* x, double* y,
     }
     rc = resident_settle(c, s);
     if (rc) return rc;
-    return resident_export(c, s, dst, false);
+    return resident_export(c, s, dst, true);      // the particles without a slot follow the cell-ordered ones
 }
 
 extern "C" int64_t ecsim_relayout_count(const ecsim_ctx* c) { return c ? c->relayouts : 0; }
@@ -670,7 +728,7 @@ extern "C" int ecsim_set_resort_fraction(ecsim_ctx* c, double fraction)
 
 extern "C" int ecsim_set_fused_warps(ecsim_ctx* c, int warps)
 {
-    if (!c || (warps != 0 && warps != 8 && warps != 12 && warps != 16)) return ECSIM_ERR_INVALID_ARG;
+    if (!c || (warps != 0 && warps != 8 && warps != 12 && warps != 16 && warps != 13 && warps != 17)) return ECSIM_ERR_INVALID_ARG;
     c->fused_warps = warps;
     return ECSIM_OK;
 }
@@ -720,18 +778,18 @@ extern "C" int64_t ecsim_leaver_count(ecsim_ctx* c)
     return total;
 }
 
-template <int NW, int REGS, int MODE, int LAYOUT>
+template <int NW, int REGS, int MODE, int LAYOUT, bool EARLY = false>
 static cudaError_t launch_fused(const ecsim_ctx* c, const FusedArgs& fa)
 {
     const size_t smem = (size_t)NW * (MODE == MODE_PUSH ? FLD_DOUBLES : WARP_SMEM_DOUBLES) * sizeof(double);
     // per launch, not per process: a second device of the same process needs its own opt-in
-    cudaError_t e = cudaFuncSetAttribute(k_fused_push_moments<NW, REGS, MODE, LAYOUT>,
+    cudaError_t e = cudaFuncSetAttribute(k_fused_push_moments<NW, REGS, MODE, LAYOUT, EARLY>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const size_t cells = (size_t)(fa.c_end - fa.c_begin);
     size_t grid = (cells + NW - 1) / NW;
     if (grid > (size_t)c->sm_count) grid = (size_t)c->sm_count;
-    k_fused_push_moments<NW, REGS, MODE, LAYOUT><<<(int)grid, NW * 32, smem, c->stream>>>(fa);
+    k_fused_push_moments<NW, REGS, MODE, LAYOUT, EARLY><<<(int)grid, NW * 32, smem, c->stream>>>(fa);
     return cudaGetLastError();
 }
 
@@ -761,6 +819,8 @@ static cudaError_t launch_fused_any(const ecsim_ctx* c, const FusedArgs& fa, int
     if (mode == MODE_MOMENTS)
         return gapped ? launch_fused<12, 168, MODE_MOMENTS, LAYOUT_GAPPED>(c, fa) : launch_fused<12, 168, MODE_MOMENTS, LAYOUT_DENSE>(c, fa);
     if (gapped) return launch_fused<12, 168, MODE_FUSED, LAYOUT_GAPPED>(c, fa);
+    if (c->fused_warps == 13) return launch_fused<12, 168, MODE_FUSED, LAYOUT_DENSE, true>(c, fa);   // experiment: early fetch
+    if (c->fused_warps == 17) return launch_fused<16, 128, MODE_FUSED, LAYOUT_DENSE, true>(c, fa);
     if (c->fused_warps == 8) return launch_fused<8, 224, MODE_FUSED, LAYOUT_DENSE>(c, fa);
     if (c->fused_warps == 16) return launch_fused<16, 128, MODE_FUSED, LAYOUT_DENSE>(c, fa);
     return launch_fused<12, 168, MODE_FUSED, LAYOUT_DENSE>(c, fa);
@@ -827,10 +887,11 @@ static int fill_fused_args(ecsim_ctx* c, FusedArgs& fa, int n_list, const int* l
             d.seg = r.seg; d.Fin = r.F[r.cur]; d.Rin = r.R[r.cur]; d.Fout = r.F[1 - r.cur]; d.Rout = r.R[1 - r.cur];
             d.x = in[0]; d.y = in[1]; d.z = in[2]; d.u = in[3]; d.v = in[4]; d.w = in[5]; d.q = in[6];
             d.ox = out[0]; d.oy = out[1]; d.oz = out[2]; d.ou = out[3]; d.ov = out[4]; d.ow = out[5]; d.oq = out[6];
-            d.ovf = r.ovf; d.ovf_cap = r.ovf_cap; d.ovf_count = r.ovf_count;
+            d.ovf = r.ovf[1 - r.ovf_cur]; d.ovf_cap = r.ovf_cap; d.ovf_count = r.ovf_count[1 - r.ovf_cur];
             if (push) {
                 CK(cudaMemsetAsync(d.Rout, 0, sizeof(uint32_t) * cells, c->stream));
-                c->launches++;
+                CK(cudaMemsetAsync(d.ovf_count, 0, sizeof(uint32_t), c->stream));
+                c->launches += 2;
             }
         } else {
             d.seg = w.start + (size_t)s * (cells + 1);
@@ -918,6 +979,20 @@ static int step_impl(ecsim_ctx* c, int mode, int n_list, const int* list, const 
     }
     if (c->timing) { CK(cudaEventRecord(c->ev1, c->stream)); c->ev_valid = true; }
 
+    // resident species: the particles without a slot (overflow list of the last push) -- deposit, push, try again for a slot
+    if (gapped) {
+        for (int i = 0; i < n_list; ++i) {
+            SpeciesHost& sp = c->sp[list[i]];
+            Resident& r = sp.res;
+            HomelessArgs a;
+            a.g = g; a.sp = fa.sp[i]; a.in = r.ovf[r.ovf_cur]; a.in_cap = r.ovf_cap; a.in_count = r.ovf_count[r.ovf_cur];
+            a.E = fa.E; a.B = B; a.dt = dt; a.AM = w.AM;
+            a.do_deposit = deposit ? 1 : 0; a.do_push = push ? 1 : 0;
+            k_push_homeless<<<c->sm_count * 4, STRAY_WARPS * 32, 0, c->stream>>>(a);
+            CK_LAUNCH();
+            c->launches++;
+        }
+    }
     // strays (dense layout only): each is added to the per-cell accumulators of its true cell with one bulk reduction
     // (a 2.2 KB block instead of atomics on eight node blocks), then one expansion serves everybody
     if (!gapped) {
@@ -959,8 +1034,9 @@ static int step_impl(ecsim_ctx* c, int mode, int n_list, const int* list, const 
         if (push) {
             CK(cudaMemcpyAsync(c->h_leavers + s, w.leavers + s, sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
             if (gapped) {
-                CK(cudaMemcpyAsync(c->h_ovf + s, sp.res.ovf_count, sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream));
-                sp.res.cur = 1 - sp.res.cur;            // the species now lives in the buffer just written
+                sp.res.cur = 1 - sp.res.cur;            // the species now lives in the buffer just written,
+                sp.res.ovf_cur = 1 - sp.res.ovf_cur;    // its homeless particles in the list just written
+                CK(cudaMemcpyAsync(c->h_ovf + s, sp.res.ovf_count[sp.res.ovf_cur], sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream));
             }
             CK(cudaEventRecord(sp.leavers_event, c->stream));
             sp.leavers_pending = true;
@@ -1043,7 +1119,7 @@ extern "C" int ecsim_diagnostics(ecsim_ctx* c, int species, double* rho, double*
         if (sp.n > 0) {
             k_iota_u32<<<grid_for(c, (size_t)sp.n, 256, 16), 256, 0, c->stream>>>((uint32_t)sp.n, w.perm, w.stray_count + species);
             CK_LAUNCH();
-            DiagStrayArgs a{g, w.perm, w.stray_count + species, sp.x, sp.y, sp.z, sp.u, sp.v, sp.w, sp.q, rho, J, P, Q};
+            DiagStrayArgs a{g, w.perm, w.stray_count + species, 0xffffffffu, sp.x, sp.y, sp.z, sp.u, sp.v, sp.w, sp.q, rho, J, P, Q};
             k_diag_strays<<<grid_for(c, (size_t)sp.n, 128, 16), 128, 0, c->stream>>>(a);
             CK_LAUNCH();
             c->launches += 2;
@@ -1065,7 +1141,17 @@ extern "C" int ecsim_diagnostics(ecsim_ctx* c, int species, double* rho, double*
     CK_LAUNCH();
     c->launches++;
     if (!gapped && sp.n > 0) {
-        DiagStrayArgs a{g, fa.sp[0].stray_list, fa.sp[0].stray_count, sp.x, sp.y, sp.z, sp.u, sp.v, sp.w, sp.q, rho, J, P, Q};
+        DiagStrayArgs a{g, fa.sp[0].stray_list, fa.sp[0].stray_count, 0xffffffffu, sp.x, sp.y, sp.z, sp.u, sp.v, sp.w, sp.q, rho, J, P, Q};
+        k_diag_strays<<<c->sm_count * 2, 128, 0, c->stream>>>(a);
+        CK_LAUNCH();
+        c->launches++;
+    }
+    if (gapped) {
+        // the particles without a slot: straight from the overflow list (list = identity)
+        const Resident& r = sp.res;
+        const double* o = r.ovf[r.ovf_cur];
+        const size_t m = r.ovf_cap;
+        DiagStrayArgs a{g, nullptr, r.ovf_count[r.ovf_cur], r.ovf_cap, o, o + m, o + 2 * m, o + 3 * m, o + 4 * m, o + 5 * m, o + 6 * m, rho, J, P, Q};
         k_diag_strays<<<c->sm_count * 2, 128, 0, c->stream>>>(a);
         CK_LAUNCH();
         c->launches++;

@@ -241,6 +241,7 @@ __device__ __forceinline__ bool phase1(const Geom& g, const ParticleRegs& r, boo
         const double vbz = a20 * tx + a21 * ty + a22 * tz;
         out.u = 2.0 * vbx - vx; out.v = 2.0 * vby - vy; out.w = 2.0 * vbz - vz;
         double xn = fma(dt, out.u, r.x), yn = fma(dt, out.v, r.y), zn = fma(dt, out.w, r.z);
+        pin_axes(g, xn, yn, zn);        // reduced dimensionality (L123 fixPosition); a warp-uniform no-op in 3-D
         // for x >= +0 the order of doubles is the order of their bit patterns: "0 <= x < L" is one unsigned compare
         const bool in_box = (unsigned long long)__double_as_longlong(xn) < (unsigned long long)__double_as_longlong(g.Lx) &&
                             (unsigned long long)__double_as_longlong(yn) < (unsigned long long)__double_as_longlong(g.Ly) &&
@@ -323,7 +324,7 @@ __device__ __forceinline__ void relocate(const Geom& g, const SpeciesDev& sp, co
 
 // REGS: register cap.  Measured on config 2 (whole grid, ms): 12 warps x 168 regs 11.89, 12 x 144 12.23, 16 x 128
 // 12.15, 12 x 128 12.88, 8 x 200 13.63; warp counts that are not a multiple of the 4 schedulers lose (14 x 128 13.58).
-template <int NW, int REGS, int MODE, int LAYOUT>
+template <int NW, int REGS, int MODE, int LAYOUT, bool EARLY = false>
 __global__ void __maxnreg__(REGS)
 k_fused_push_moments(const __grid_constant__ FusedArgs a)
 {
@@ -492,6 +493,12 @@ k_fused_push_moments(const __grid_constant__ FusedArgs a)
                 }
             }
 
+            // EARLY: the next batch's loads are requested before this batch's phase 1 (more time to land, 14 more live registers)
+            if (EARLY) {
+                if (in_state == 1 || in_state == 2) fetch();
+                if (in_state != 1 && has_next) { load_fields(ni, nj, nk, f0, f1); fld_ready = true; }
+            }
+
             // ---- phase 1: lane = particle ----
             PushedRegs o;
             const bool active = lane < nb;
@@ -516,8 +523,10 @@ k_fused_push_moments(const __grid_constant__ FusedArgs a)
                 }
             }
             // global loads of the next batch fly during phase 2
-            if (in_state == 1 || in_state == 2) fetch();
-            if (in_state != 1 && has_next) { load_fields(ni, nj, nk, f0, f1); fld_ready = true; }
+            if (!EARLY) {
+                if (in_state == 1 || in_state == 2) fetch();
+                if (in_state != 1 && has_next) { load_fields(ni, nj, nk, f0, f1); fld_ready = true; }
+            }
             if (!GAPPED) {
                 const unsigned smask = __ballot_sync(0xffffffffu, active && !inside);
                 if (smask) {

@@ -286,6 +286,10 @@ k_fused_ws(const __grid_constant__ FusedArgs a)
                 }
             }
             const bool end_species = in_state != 1 || in_s != s, end_cell = in_state != 1;
+            // the next batch's particles (and the next cell's corner fields) are requested BEFORE this batch's phase 1:
+            // the producer has no phase 2 to hide the loads behind
+            if (in_state == 1 || in_state == 2) fetch();
+            if (in_state != 1 && has_next) { load_fields(ni, nj, nk, f0, f1); fld_ready = true; }
 
             // ---- phase 1 into the pair's free tile ----
             const int t = (int)(b & 1u);
@@ -313,8 +317,6 @@ k_fused_ws(const __grid_constant__ FusedArgs a)
                     my_leavers += o.stays ? 0u : 1u;
                 }
             }
-            if (in_state == 1 || in_state == 2) fetch();
-            if (in_state != 1 && has_next) { load_fields(ni, nj, nk, f0, f1); fld_ready = true; }
             if (!GAPPED) {
                 const unsigned smask = __ballot_sync(0xffffffffu, active && !inside);
                 if (smask) {

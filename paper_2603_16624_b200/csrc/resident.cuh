@@ -12,16 +12,17 @@
 struct Soa7 { double* a[7]; };
 struct Soa7c { const double* a[7]; };
 
-// slots of cell c = its particles + max(min_slack, ceil(slack * particles)), rounded up to a multiple of 4 (32-byte
-// sector alignment of every segment)
+// slots of cell c = its particles + max(min_slack, ceil(slack * max(particles, mean particles per cell))), rounded up to a
+// multiple of 4 (32-byte sector alignment of every segment).  The mean enters because the arrivals of a step scale with
+// the population of the NEIGHBOURHOOD, not of the cell itself: a depleted cell beside a dense one needs room too.
 __global__ void __launch_bounds__(256)
-k_gapped_caps(uint32_t cells, const uint32_t* __restrict__ count, double slack, uint32_t min_slack,
+k_gapped_caps(uint32_t cells, const uint32_t* __restrict__ count, double slack, uint32_t min_slack, double mean,
               uint32_t* __restrict__ cap)
 {
     const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= cells) return;
     const uint32_t n = count[c];
-    uint32_t extra = (uint32_t)ceil(slack * (double)n);
+    uint32_t extra = (uint32_t)ceil(slack * fmax((double)n, mean));
     if (extra < min_slack) extra = min_slack;
     cap[c] = (n + extra + 3u) & ~3u;
 }

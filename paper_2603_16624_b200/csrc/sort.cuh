@@ -244,6 +244,18 @@ k_stage_to_slots(uint32_t n, const uint32_t* __restrict__ dest, const uint32_t* 
     for (uint32_t t = threadIdx.x; t < tile_n; t += SORT_STAGE_THREADS) tmp[dsts[t]] = vals[t];
 }
 
+// fixPosition on stored particles (L123): pin the masked coordinates of n slots (set-up of a reduced-dimension run)
+__global__ void __launch_bounds__(256)
+k_fix_position(Geom g, size_t n, double* __restrict__ x, double* __restrict__ y, double* __restrict__ z)
+{
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += stride) {
+        if (g.fix_mask & 1) x[p] = g.fix_pos[0];
+        if (g.fix_mask & 2) y[p] = g.fix_pos[1];
+        if (g.fix_mask & 4) z[p] = g.fix_pos[2];
+    }
+}
+
 // list[i] = i, *count = n ("every particle" as a list, for kernels that take one)
 __global__ void __launch_bounds__(256)
 k_iota_u32(uint32_t n, uint32_t* __restrict__ list, uint32_t* __restrict__ count)

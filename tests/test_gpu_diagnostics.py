@@ -107,3 +107,33 @@ def test_diagnostics_null_outputs_and_ragged_grid():
     assert np.all(np.abs(got[2].cpu().numpy() - d.P) <= MOM_TOL * d.P_abs)
     assert bool(torch.isnan(got[0]).all()) and bool(torch.isnan(got[1]).all()) and bool(torch.isnan(got[3]).all())
     ctx.close()
+
+
+def test_diagnostics_of_a_resident_species_with_homeless_particles():
+    """Segments without slack and hot particles: some particles sit in the overflow list; the diagnostics count them."""
+    import dataclasses
+    base = wl.config(0, (6, 6, 6))
+    hot = tuple(dataclasses.replace(sp, vth=v) for sp, v in zip(base.species, (1.0, 0.5)))
+    cfg = dataclasses.replace(base, dt=0.2, ppc=40, species=hot)
+    E, B, parts = gen_all(cfg)
+    pcs = [to_cuda(p) for p in parts]
+    ctx = make_ctx(cfg, max(p["n"] for p in parts))
+    ctx.set_resort_fraction(100.0)
+    for s, sp in enumerate(cfg.species):
+        ctx.load_particles(s, sp.qom, pcs[s], sorted=True)
+        ctx.make_resident(s, 0.0)
+    rho, J, M = alloc_moments(cfg.nodes, 2)
+    for _ in range(2):
+        ctx.push_and_moments_all(E, B, cfg.dt, cfg.theta, rho, J, M)
+    torch.cuda.synchronize()
+    assert ctx.relayout_count() == 0
+    for s in range(2):
+        cur = {k: torch.empty_like(pcs[s][k]) for k in PKEYS}
+        ctx.export_particles(s, cur)
+        got = _alloc(cfg.nodes)
+        ctx.diagnostics(s, *got)
+        torch.cuda.synchronize()
+        d = oracle.Diagnostics(cfg.nodes)
+        oracle.diagnostics(grid_of(cfg), {k: cur[k].cpu().numpy() for k in PKEYS}, d)
+        _check(got, d, f"species {s}")
+    ctx.close()

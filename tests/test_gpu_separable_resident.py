@@ -140,13 +140,15 @@ def test_separable_calls_with_strays_dense():
 
 # ------------------------------------------------------------------ resident species: the sort-preserving push
 
-def _resident_run(cfg, steps, slack, mode, E, B, parts_np, expect_relayout=None):
+def _resident_run(cfg, steps, slack, mode, E, B, parts_np, expect_relayout=None, resort_fraction=None):
     """`mode`: 'fused' (ecsim_push_and_moments_all), 'split' (moments_all + push_all) or 'single' (per-species calls)."""
     nsp = len(cfg.species)
     q0 = [sp.q_sign * cfg.q_abs for sp in cfg.species]
     n_s = [p["x"].shape[0] for p in parts_np]
     parts_cuda = [to_cuda(from_numpy(p)) for p in parts_np]
     ctx = make_ctx(cfg, max(n_s + [1]))
+    if resort_fraction is not None:
+        ctx.set_resort_fraction(resort_fraction)
     for s, sp in enumerate(cfg.species):
         ctx.load_particles(s, sp.qom, parts_cuda[s], sorted=False)
         ctx.make_resident(s, slack)
@@ -242,15 +244,20 @@ def test_resident_harris_sheet_and_shuffled_input():
     _resident_run(cfg, 4, 0.25, "fused", E.cuda(), B.cuda(), parts_np)
 
 
-def test_resident_overflow_forces_a_fresh_layout():
+@pytest.mark.parametrize("resort_fraction", [0.0, 100.0], ids=["fresh_layout", "homeless_forever"])
+def test_resident_full_segments(resort_fraction):
     """Hot particles (a quarter of them change cell per step) and segments with next to no slack: arrivals find their new
-    cell full, go to the overflow list, and the next call lays the species out afresh.  Same parity throughout."""
+    cell full and go to the overflow list.  Every later pass deposits and pushes those homeless particles one warp each
+    and tries again for a slot; with resort_fraction = 0 any overflow makes the next call lay the species out afresh,
+    with 100 it never does.  Same parity either way (diagnostics included)."""
     base = wl.config(0, (6, 6, 6))
     hot = tuple(dataclasses.replace(sp, vth=v) for sp, v in zip(base.species, (1.0, 0.5)))
     cfg = dataclasses.replace(base, dt=0.2, ppc=40, species=hot)
     E, B = wl.gen_fields(cfg)
-    leavers = _resident_run(cfg, 5, 0.0, "fused", E.cuda(), B.cuda(), _tagged_parts(cfg), expect_relayout=True)
+    leavers = _resident_run(cfg, 5, 0.0, "fused", E.cuda(), B.cuda(), _tagged_parts(cfg),
+                            expect_relayout=(resort_fraction == 0.0), resort_fraction=resort_fraction)
     assert leavers > 1000
+    _resident_run(cfg, 3, 0.0, "split", E.cuda(), B.cuda(), _tagged_parts(cfg), resort_fraction=resort_fraction)
 
 
 def test_resident_ragged_random_grid_three_species():

@@ -452,3 +452,29 @@ def test_config0_invariants():
     lhs = ((mom.J + ME) * E).sum() * cfg.dx * cfg.dy * cfg.dz
     # global energy identity: field work = kinetic energy change / dt
     assert abs(lhs - rhs) < 1e-9 * (np.abs(mom.J_abs * E).sum() + np.abs(ME * E).sum())
+
+
+def test_all_cores_timing_variant_equals_the_oracle():
+    """oracle.step_planes (the all-host-cores timing variant bench.py reports beside the GPU number) has no arithmetic of
+    its own -- it calls oracle.step per x-plane of cells, even planes in parallel, then odd planes -- so it must agree
+    with the sequential oracle up to the per-node summation order: <= 1e-12 of the |addend| sums; particles bitwise."""
+    import workloads as wl
+    from util import grid_of, to_numpy
+    for scale in ((6, 5, 4), (7, 4, 3)):                       # even and odd nx (odd: the last plane runs alone)
+        cfg = wl.config(0, scale)
+        E, B = wl.gen_fields(cfg)
+        En, Bn = E.numpy(), B.numpy()
+        for s, sp in enumerate(cfg.species):
+            p = to_numpy(wl.gen_species(cfg, s))
+            count, start = wl.cell_layout(cfg)
+            plane_start = start.numpy()[::cfg.ny * cfg.nz].copy()
+            a, b = {k: v.copy() for k, v in p.items()}, {k: v.copy() for k, v in p.items()}
+            ma, mb = oracle.Moments(cfg.nodes), oracle.Moments(cfg.nodes, with_abs=False)
+            oracle.step(grid_of(cfg), sp.qom, cfg.dt, a, En, Bn, ma)
+            oracle.step_planes(grid_of(cfg), sp.qom, cfg.dt, b, plane_start, En, Bn, mb)
+            for k in "xyzuvw":
+                assert np.array_equal(a[k], b[k])
+            assert np.all(np.abs(ma.rho - mb.rho) <= 1e-12 * ma.rho_abs)
+            assert np.all(np.abs(ma.J - mb.J) <= 1e-12 * ma.J_abs)
+            assert np.all(np.abs(ma.M - mb.M) <= 1e-12 * ma.M_abs)
+    assert oracle.threads() >= 1

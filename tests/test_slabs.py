@@ -1,0 +1,140 @@
+"""Slab domain decomposition (paper_2603_16624_b200/slabs.py) WITHOUT a GPU:
+  * all ranks in one process (LocalRing): even and uneven splits, world = 1 (self-exchange = the periodic wrap), 3 steps
+    with halo add + migration after every step, against the single-domain oracle;
+  * two real ranks over torch.distributed / gloo (the N > 1 path the tier asks to cover on CPU).
+The per-slab compute engine here is the CPU oracle on the slab's local grid; tests/test_gpu_slabs.py runs libecpush."""
+from __future__ import annotations
+
+import os
+import socket
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+import torch
+
+import workloads as wl
+from paper_2603_16624_b200.slabs import PKEYS, LocalRing, SlabGrid
+from slab_driver import (check_against_global, global_reference_step, oracle_engine, tagged_global_particles)
+from util import grid_of
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def run_local_ring(cfg, world, steps, engine):
+    E, B = wl.gen_fields(cfg)
+    gparts = tagged_global_particles(cfg)
+    ref = [{k: p[k].numpy().copy() for k in PKEYS} for p in gparts]
+    grids = [SlabGrid(*grid_of(cfg), world, r) for r in range(world)]
+    ring = LocalRing(world)
+    parts = [[g.split_particles(p) for p in gparts] for g in grids]
+    fields = [(g.local_fields(E), g.local_fields(B)) for g in grids]
+    nsp = len(cfg.species)
+    moved = 0
+    for step in range(steps):
+        out = [engine(grids[r], cfg, parts[r], *fields[r]) for r in range(world)]
+        halos = [grids[r].halo_planes(*out[r]) for r in range(world)]
+        got = ring.shift_right(halos)
+        for r in range(world):
+            grids[r].add_halo(got[r], *out[r])
+        for s in range(nsp):
+            packs = [grids[r].leavers(parts[r][s]) for r in range(world)]
+            fl, fr = ring.exchange([p[1] for p in packs], [p[2] for p in packs])
+            moved += sum(int(p[1].shape[1] + p[2].shape[1]) for p in packs)
+            for r in range(world):
+                parts[r][s] = grids[r].merge(parts[r][s], packs[r][0], fl[r], fr[r])
+        per, total = global_reference_step(cfg, ref, E, B)
+        check_against_global(cfg, grids, [grids[r].owned(out[r][0], 1) for r in range(world)],
+                             [grids[r].owned(out[r][1], 2) for r in range(world)],
+                             [grids[r].owned(out[r][2], 0) for r in range(world)],
+                             [[grids[r].to_global(parts[r][s]) for s in range(nsp)] for r in range(world)], ref, per, total,
+                             f"world {world} step {step}")
+    return moved
+
+
+@pytest.mark.parametrize("world", [1, 2, 3])
+def test_slabs_in_one_process_match_the_single_domain_oracle(world):
+    import dataclasses
+    base = wl.config(0, (8, 5, 4))
+    hot = tuple(dataclasses.replace(sp, vth=v) for sp, v in zip(base.species, (1.5, 0.5)))   # plenty of slab crossings
+    cfg = dataclasses.replace(base, species=hot, ppc=12, dt=0.2)
+    moved = run_local_ring(cfg, world, 3, oracle_engine)
+    assert moved > 50
+
+
+def test_slab_grid_bookkeeping():
+    g = [SlabGrid(10, 3, 2, 0.5, 1.0, 1.0, 3, r) for r in range(3)]
+    assert [(s.i0, s.i1) for s in g] == [(0, 3), (3, 6), (6, 10)]
+    assert g[0].left == 2 and g[0].right == 1 and g[0].nxl_left == 4
+    assert g[2].local_dims[:3] == (6, 3, 2)
+    F = torch.arange(3 * 60, dtype=torch.float64).reshape(3, 60)
+    Fl = g[2].local_fields(F).reshape(3, 6, 6)
+    G = F.reshape(3, 10, 6)
+    for l, gi in enumerate([6, 7, 8, 9, 0, 5]):                 # planes 0..nxl = 6..9, 0 (right halo); plane nxl+1 = 5 (left)
+        assert torch.equal(Fl[:, l], G[:, gi])
+    with pytest.raises(ValueError):
+        SlabGrid(2, 3, 3, 1.0, 1.0, 1.0, 3, 0)
+
+
+WORKER = r'''
+import os, sys
+root = os.environ["ECPUSH_ROOT"]
+sys.path[:0] = [root, os.path.join(root, "tests")]
+import dataclasses
+import numpy as np, torch, torch.distributed as dist
+import workloads as wl
+from paper_2603_16624_b200.slabs import PKEYS, DistRing, SlabGrid
+from slab_driver import check_against_global, global_reference_step, oracle_engine, tagged_global_particles
+from util import grid_of
+
+dist.init_process_group("gloo")
+rank, world = dist.get_rank(), dist.get_world_size()
+base = wl.config(0, (8, 5, 4))
+hot = tuple(dataclasses.replace(sp, vth=v) for sp, v in zip(base.species, (1.5, 0.5)))
+cfg = dataclasses.replace(base, species=hot, ppc=12, dt=0.2)
+E, B = wl.gen_fields(cfg)
+gparts = tagged_global_particles(cfg)
+grid = SlabGrid(*grid_of(cfg), world, rank)
+ring = DistRing()
+parts = [grid.split_particles(p) for p in gparts]
+El, Bl = grid.local_fields(E), grid.local_fields(B)
+ref = [{k: p[k].numpy().copy() for k in PKEYS} for p in gparts]
+nsp = len(cfg.species)
+for step in range(3):
+    rho, J, M = oracle_engine(grid, cfg, parts, El, Bl)
+    grid.add_halo(ring.shift_right(grid.halo_planes(rho, J, M)), rho, J, M)
+    for s in range(nsp):
+        stay, pr, pl = grid.leavers(parts[s])
+        fl, fr = ring.exchange(pr, pl)
+        parts[s] = grid.merge(parts[s], stay, fl, fr)
+    mine = (grid.owned(rho, 1).clone(), grid.owned(J, 2).clone(), grid.owned(M, 0).clone(),
+            [{k: v.numpy() for k, v in grid.to_global(parts[s]).items()} for s in range(nsp)])
+    gathered = [None] * world
+    dist.gather_object(mine, gathered if rank == 0 else None, dst=0)
+    if rank == 0:
+        grids = [SlabGrid(*grid_of(cfg), world, r) for r in range(world)]
+        per, total = global_reference_step(cfg, ref, E, B)
+        check_against_global(cfg, grids, [g[0] for g in gathered], [g[1] for g in gathered], [g[2] for g in gathered],
+                             [g[3] for g in gathered], ref, per, total, f"gloo step {step}")
+dist.barrier()
+dist.destroy_process_group()
+print(f"rank {rank} ok")
+'''
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def test_two_gloo_ranks_halo_add_and_migration(tmp_path):
+    script = tmp_path / "slab_worker.py"
+    script.write_text(WORKER)
+    env = dict(os.environ, ECPUSH_ROOT=ROOT)
+    out = subprocess.run(
+        [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2", "--master-addr", "127.0.0.1",
+         "--master-port", str(_free_port()), str(script)], env=env, capture_output=True, text=True, timeout=600)
+    assert out.returncode == 0, out.stdout + out.stderr
+    assert "rank 0 ok" in out.stdout and "rank 1 ok" in out.stdout
