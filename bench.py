@@ -39,9 +39,26 @@ BYTES_PER_PARTICLE_CFG2 = 119.8
 # FP64 vector peak derived from unit counts and clocks: 148 SM x 64 FMA/clk x 2 flop x 1.965 GHz
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 NORTH_STAR_ROOFLINE_PPS = min(8.0e12 / BYTES_PER_PARTICLE_CFG2, FP64_PEAK_TFLOPS * 1e12 / FLOP_PER_PARTICLE)
-# dram__bytes_read.sum + dram__bytes_write.sum of k_fused_push_moments per launch, from the ncu
-# --set full capture summarised in profiles/ (None until a capture of this workload exists)
-FUSED_DRAM_TRAFFIC_BYTES = 33.50e9   # profiles/r01c: 15.50 GB read + 18.00 GB written per launch on configs[2]
+
+
+def profiled_traffic(kernel_substring: str, launch_list_glob: str = "profiles/r*_launches_cfg2.csv"):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of a kernel, read from the newest COMMITTED ncu launch list
+    of the headline workload (profiles/rNN?_launches_cfg2.csv, written by the command named in the README beside it).
+    Returns (bytes, file) or (None, None): never a constant typed into this file."""
+    import csv
+    import glob
+    for path in sorted(glob.glob(os.path.join(ROOT, launch_list_glob)), reverse=True):
+        per_launch = {}
+        try:
+            for r in csv.reader(open(path)):
+                if len(r) > 14 and kernel_substring in r[4] and r[12] in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+                    per_launch.setdefault(r[0], {})[r[12]] = float(r[14].replace(",", ""))
+        except (OSError, ValueError):
+            continue
+        full = [v["dram__bytes_read.sum"] + v["dram__bytes_write.sum"] for v in per_launch.values() if len(v) == 2]
+        if full:
+            return sum(full) / len(full), os.path.relpath(path, ROOT)
+    return None, None
 
 
 def parse_args():
@@ -313,6 +330,9 @@ def run_product(args):
     k_ms = sum(kernel_ms) / len(kernel_ms)
     achieved_tflops = FLOP_PER_PARTICLE * n_total / (k_ms * 1e-3) / 1e12
 
+    traffic, traffic_src = (None, None)
+    if args.variant == "fused" and cfg.idx == 2 and not args.scale:
+        traffic, traffic_src = profiled_traffic("k_fused_push_moments<12, 168, 0, 0")
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -328,7 +348,7 @@ def run_product(args):
         "roofline": {
             "bound": "alu", "kernel": "k_fused_push_moments" if args.variant == "fused" else "k_push_moments_atomic",
             "achieved": achieved_tflops, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved_tflops / FP64_PEAK_TFLOPS,
-            "traffic": FUSED_DRAM_TRAFFIC_BYTES if (args.variant == "fused" and cfg.idx == 2 and not args.scale) else None,
+            "traffic": traffic, "traffic_source": traffic_src,
             "peak_source": "derived: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md); fp64_probe_tflops is the DFMA "
                            "micro-benchmark measured in this run",
             "fp64_probe_tflops": fp64_probe, "kernel_ms": k_ms, "flop_per_particle": FLOP_PER_PARTICLE,

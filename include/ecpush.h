@@ -203,6 +203,17 @@ int ecsim_apply_M(ecsim_ctx *ctx, const double *M, const double *E, double *out,
  * workspace, which must be ecsim_host_step_workspace_bytes() large), runs the step, copies particles
  * and moments back, and synchronises the stream.  Host arrays: x..w in/out [n], q in [n], E/B in,
  * rho/Jhat/M out (with accumulate != 0 the accumulated arrays are copied in first).  Pinned host memory makes the copies asynchronous. */
+/* When the arrays are declared cell-sorted (sorted != 0, accumulate = 0, variant FUSED) the step runs as a pipeline over
+ * slabs of x-planes on three streams -- upload slab k+1 | bin, deposit + push, expand slab k | download slab k-1 -- so
+ * that the two directions of the PCIe link overlap (one cudaMemcpyAsync per array per slab; pinned host memory is
+ * needed for the overlap, pageable memory still gives the right result).  For these two host entries `sorted` != 0 is
+ * therefore a CONTRACT, not a hint: if a particle is found outside the slab / cell its place in the arrays implies, the
+ * call returns ECSIM_ERR_INVALID_ARG (text in ecsim_last_error) and the particle arrays are left partially advanced.
+ * Pass sorted = 0 when unsure (serial path, the library sorts).  ecsim_set_host_pipeline(0) forces the serial path, (2)
+ * pipelines even tiny inputs (default 1: only when a slab carries >= 32 MB); ecsim_host_pipelined_count = calls that
+ * completed through the pipeline. */
+int ecsim_set_host_pipeline(ecsim_ctx *ctx, int on);
+int64_t ecsim_host_pipelined_count(const ecsim_ctx *ctx);
 size_t ecsim_host_step_workspace_bytes(const ecsim_ctx *ctx, int64_t n_particles);
 int ecsim_push_and_moments_host(ecsim_ctx *ctx, int64_t n, double q_over_m, int sorted,
                                 double *x, double *y, double *z, double *u, double *v, double *w,

@@ -62,6 +62,8 @@ _PROTOS = {
     "ecsim_make_resident": (_c.c_int, [_P, _c.c_int, _P, _c.c_size_t, _c.c_double]),
     "ecsim_export_particles": (_c.c_int, [_P, _c.c_int] + [_P] * 7),
     "ecsim_relayout_count": (_c.c_int64, [_P]),
+    "ecsim_set_host_pipeline": (_c.c_int, [_P, _c.c_int]),
+    "ecsim_host_pipelined_count": (_c.c_int64, [_P]),
     "ecsim_apply_M": (_c.c_int, [_P, _P, _P, _P, _c.c_int]),
     "ecsim_diagnostics": (_c.c_int, [_P, _c.c_int, _P, _P, _P, _P]),
     "ecsim_set_fixed_axes": (_c.c_int, [_P, _c.c_int, _c.c_double, _c.c_double, _c.c_double]),
@@ -241,6 +243,12 @@ class Ecsim:
         f64 = self.torch.float64
         ptrs = [_dptr(out[k], f64) for k in ("x", "y", "z", "u", "v", "w", "q")]
         _check(self.L.ecsim_export_particles(self.h, species, *ptrs), "ecsim_export_particles")
+
+    def set_host_pipeline(self, mode: int):
+        _check(self.L.ecsim_set_host_pipeline(self.h, int(mode)), "ecsim_set_host_pipeline")
+
+    def host_pipelined_count(self) -> int:
+        return int(self.L.ecsim_host_pipelined_count(self.h))
 
     def relayout_count(self) -> int:
         return int(self.L.ecsim_relayout_count(self.h))

@@ -38,6 +38,7 @@ static int cuda_fail(cudaError_t e, const char* what, int line)
 #define CK_LAUNCH() CK(cudaGetLastError())
 
 enum SortState { ST_UNSORTED = 0, ST_DECLARED = 1, ST_SEGMENTED = 2 };
+#define ECSIM_HOST_SLABS_MAX 32
 
 // A RESIDENT species (ecsim_make_resident): library-managed gapped double buffers in memory the caller lent
 // (resident.cuh; LAYOUT_GAPPED of fused_mma.cuh).
@@ -115,6 +116,12 @@ struct ecsim_ctx {
     int64_t resorts = 0;
     int64_t relayouts = 0;
     int m_layout = ECSIM_M_27;
+    // pipelined host step: upload / download streams beside the caller's stream, one event pair per slab
+    cudaStream_t s_up = nullptr, s_down = nullptr;
+    cudaEvent_t ev_up[ECSIM_HOST_SLABS_MAX] = {}, ev_comp[ECSIM_HOST_SLABS_MAX] = {}, ev_exp[ECSIM_HOST_SLABS_MAX] = {};
+    cudaEvent_t ev_start = nullptr, ev_fields = nullptr, ev_down = nullptr;
+    int host_pipeline = 1;
+    int64_t host_pipelined_calls = 0;
 };
 
 static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
@@ -224,6 +231,16 @@ extern "C" int ecsim_init_grid(ecsim_ctx** ctx, int nx, int ny, int nz, double d
     if (e == cudaSuccess) e = cudaMallocHost(&c->h_leavers, sizeof(unsigned long long) * n_species);
     if (e == cudaSuccess) e = cudaMallocHost(&c->h_strays, sizeof(uint32_t) * n_species);
     if (e == cudaSuccess) e = cudaMallocHost(&c->h_ovf, sizeof(uint32_t) * n_species);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->s_up, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->s_down, cudaStreamNonBlocking);
+    for (int k = 0; k < ECSIM_HOST_SLABS_MAX && e == cudaSuccess; ++k) {
+        e = cudaEventCreateWithFlags(&c->ev_up[k], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_comp[k], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_exp[k], cudaEventDisableTiming);
+    }
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_start, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_fields, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_down, cudaEventDisableTiming);
     if (e != cudaSuccess) {
         int rc = cuda_fail(e, "context set-up", __LINE__);
         ecsim_destroy(c);
@@ -247,6 +264,16 @@ extern "C" int ecsim_destroy(ecsim_ctx* c)
     if (c->h_leavers) cudaFreeHost(c->h_leavers);
     if (c->h_strays) cudaFreeHost(c->h_strays);
     if (c->h_ovf) cudaFreeHost(c->h_ovf);
+    for (int k = 0; k < ECSIM_HOST_SLABS_MAX; ++k) {
+        if (c->ev_up[k]) cudaEventDestroy(c->ev_up[k]);
+        if (c->ev_comp[k]) cudaEventDestroy(c->ev_comp[k]);
+        if (c->ev_exp[k]) cudaEventDestroy(c->ev_exp[k]);
+    }
+    if (c->ev_start) cudaEventDestroy(c->ev_start);
+    if (c->ev_fields) cudaEventDestroy(c->ev_fields);
+    if (c->ev_down) cudaEventDestroy(c->ev_down);
+    if (c->s_up) cudaStreamDestroy(c->s_up);
+    if (c->s_down) cudaStreamDestroy(c->s_down);
     delete c;
     return ECSIM_OK;
 }
@@ -710,6 +737,13 @@ extern "C" int ecsim_export_particles(ecsim_ctx* c, int s, double* x, double* y,
 }
 
 extern "C" int64_t ecsim_relayout_count(const ecsim_ctx* c) { return c ? c->relayouts : 0; }
+extern "C" int64_t ecsim_host_pipelined_count(const ecsim_ctx* c) { return c ? c->host_pipelined_calls : 0; }
+extern "C" int ecsim_set_host_pipeline(ecsim_ctx* c, int on)
+{
+    if (!c) return ECSIM_ERR_INVALID_ARG;
+    c->host_pipeline = on < 0 ? 0 : (on > 2 ? 2 : on);
+    return ECSIM_OK;
+}
 
 // --------------------------------------------------------------------------------------------
 extern "C" int ecsim_set_variant(ecsim_ctx* c, int variant)
@@ -1199,6 +1233,183 @@ extern "C" size_t ecsim_host_step_all_workspace_bytes(const ecsim_ctx* c, int64_
     return ecsim_workspace_bytes(c, n_max) + host_step_extra(c, n_total, c->n_species);
 }
 
+
+// ---- the pipelined form of the host step ----
+// Cell-sorted input: the particles of x-planes [i0, i1) of cells are one contiguous run of every SoA array, so the step
+// can be cut into slabs of x-planes and run as a three-stage pipeline on three streams: upload slab k+1 (H2D) | bin + fused
+// kernel + expansion of slab k (the caller's stream) | download the pushed particles and the finished node planes of
+// slab k-1 (D2H).  PCIe is full duplex, so the two copy directions overlap and the step costs about
+// max(bytes in, bytes out) / link instead of their sum.  Node plane i needs cell planes i-1 and i: slab k expands the
+// planes (i0, i1) and plane i0 (whose lower cells came with slab k-1); plane 0 waits for the last slab.  One
+// cudaMemcpyAsync per array per slab.  Returns 1 ("not applicable: take the serial path", nothing touched yet), 0 on
+// success, < 0 on errors -- among them ECSIM_ERR_INVALID_ARG when the arrays are not cell-sorted as declared.
+static uint32_t host_lower_bound_plane(const double* hx, uint32_t n, double rdx, int nx, int plane)
+{
+    uint32_t lo = 0, hi = n;
+    while (lo < hi) {
+        const uint32_t mid = lo + (hi - lo) / 2;
+        int i = (int)floor(hx[mid] * rdx);
+        i = i < 0 ? 0 : (i > nx - 1 ? nx - 1 : i);
+        if (i >= plane) hi = mid; else lo = mid + 1;
+    }
+    return lo;
+}
+
+static int host_step_pipelined(ecsim_ctx* c, int nsp, const int64_t* n, const double* qom,
+                               double* const* hp /* [nsp][7] host arrays */, const double* E_theta, const double* B,
+                               double dt, double theta, double* rho, double* Jhat, double* M, bool all_species_call,
+                               double* dpart, double* dE, double* dB, double* drho, double* dJ, double* dM)
+{
+    const Geom& g = c->g;
+    const size_t nodes = (size_t)g.nodes, plane = (size_t)g.ny * g.nz;
+    int64_t n_total = 0;
+    for (int s = 0; s < nsp; ++s) { if (n[s] <= 0) return 1; n_total += n[s]; }
+    int slabs = g.nx / 2;
+    if (slabs > ECSIM_HOST_SLABS_MAX) slabs = ECSIM_HOST_SLABS_MAX;
+    if (c->host_pipeline != 2)                                                    // (2: pipeline whatever the size -- tests)
+        while (slabs > 1 && (double)n_total * 56.0 / slabs < 32e6) --slabs;       // slabs of >= 32 MB, else one copy is as good
+    if (slabs < 2) return 1;
+    Workspace& w = c->ws;
+    const uint32_t cells = (uint32_t)nodes;
+    const size_t mper = c->m_layout == ECSIM_M_14 ? 126 : 243;
+    cudaStream_t st = c->stream, up = c->s_up, down = c->s_down;
+    // slab boundaries in every species' arrays (host binary search on the sorted x)
+    static thread_local uint32_t P[ECSIM_MAX_SPECIES][ECSIM_HOST_SLABS_MAX + 1];
+    int i_lo[ECSIM_HOST_SLABS_MAX + 1];
+    for (int k = 0; k <= slabs; ++k) i_lo[k] = (int)((long long)g.nx * k / slabs);
+    for (int s = 0; s < nsp; ++s) {
+        for (int k = 0; k < slabs; ++k) P[s][k] = host_lower_bound_plane(hp[s * 7], (uint32_t)n[s], g.rdx, g.nx, i_lo[k]);
+        P[s][slabs] = (uint32_t)n[s];
+        if (P[s][0] != 0) return 1;
+    }
+    uint32_t* bad = w.stray_count;              // (reused: the dense stray counters are reset below before they matter)
+    // device staging layout: species s at dpart + 7 * (particles before it), array a at + a * n[s]
+    size_t sp_off[ECSIM_MAX_SPECIES];
+    { size_t o = 0; for (int s = 0; s < nsp; ++s) { sp_off[s] = o; o += 7 * (size_t)n[s]; } }
+    CK(cudaEventRecord(c->ev_start, st));
+    CK(cudaStreamWaitEvent(up, c->ev_start, 0));
+    CK(cudaStreamWaitEvent(down, c->ev_start, 0));
+    CK(cudaMemcpyAsync(dE, E_theta, sizeof(double) * 3 * nodes, cudaMemcpyHostToDevice, up));
+    CK(cudaMemcpyAsync(dB, B, sizeof(double) * 3 * nodes, cudaMemcpyHostToDevice, up));
+    CK(cudaEventRecord(c->ev_fields, up));
+    CK(cudaStreamWaitEvent(st, c->ev_fields, 0));
+    CK(cudaMemsetAsync(w.count, 0, sizeof(uint32_t) * cells, st));
+    CK(cudaMemsetAsync(w.stray_count, 0, sizeof(uint32_t) * c->n_species, st));
+    CK(cudaMemsetAsync(w.leavers, 0, sizeof(unsigned long long) * c->n_species, st));
+    int list[ECSIM_MAX_SPECIES];
+    for (int s = 0; s < nsp; ++s) {
+        list[s] = s;
+        double* d = dpart + sp_off[s];
+        const size_t pn = (size_t)n[s];
+        int rc = ecsim_load_particles(c, s, n[s], qom[s], d, d + pn, d + 2 * pn, d + 3 * pn, d + 4 * pn, d + 5 * pn, d + 6 * pn, 1);
+        if (rc) return rc;
+        c->sp[s].state = ST_SEGMENTED;          // the tables are built slab by slab below
+    }
+    FusedArgs fa;
+    int rc = fill_fused_args(c, fa, nsp, list, dE, dB, dt, false, true);
+    if (rc) return rc;
+    for (int k = 0; k < slabs; ++k) {
+        const int i0 = i_lo[k], i1 = i_lo[k + 1];
+        const uint32_t c0 = (uint32_t)(i0 * plane), c1 = (uint32_t)(i1 * plane);
+        // ---- upload ----
+        for (int s = 0; s < nsp; ++s) {
+            const size_t p0 = P[s][k], cnt = (size_t)P[s][k + 1] - p0, pn = (size_t)n[s];
+            if (!cnt) continue;
+            for (int a = 0; a < 7; ++a)
+                CK(cudaMemcpyAsync(dpart + sp_off[s] + a * pn + p0, hp[s * 7 + a] + p0, sizeof(double) * cnt, cudaMemcpyHostToDevice, up));
+        }
+        CK(cudaEventRecord(c->ev_up[k], up));
+        // ---- bin, deposit + push, expand ----
+        CK(cudaStreamWaitEvent(st, c->ev_up[k], 0));
+        for (int s = 0; s < nsp; ++s) {
+            const uint32_t p0 = P[s][k], p1 = P[s][k + 1];
+            uint32_t* start = w.start + (size_t)s * (cells + 1);
+            const double* d = dpart + sp_off[s];
+            const size_t pn = (size_t)n[s];
+            if (s > 0) CK(cudaMemsetAsync(w.count + c0, 0, sizeof(uint32_t) * (c1 - c0), st));
+            if (p1 > p0) {
+                k_cell_hist_range<<<grid_for(c, (size_t)(p1 - p0), 256, 16), 256, 0, st>>>(g, p0, p1, d, d + pn, d + 2 * pn, w.count, c0, c1, bad + s);
+                CK_LAUNCH();
+            }
+            rc = scan_u32(c, w.count + c0, start + c0, c1 - c0);
+            if (rc) return rc;
+            k_add_u32<<<(c1 - c0 + 1 + 255) / 256, 256, 0, st>>>(start + c0, c1 - c0 + 1, p0);
+            CK_LAUNCH();
+            c->launches += 2;
+        }
+        fa.c_begin = c0; fa.c_end = c1;
+        cudaError_t e = launch_fused_any(c, fa, MODE_FUSED, false);
+        if (e != cudaSuccess) return cuda_fail(e, "k_fused_push_moments launch (host pipeline)", __LINE__);
+        c->launches++;
+        CK(cudaEventRecord(c->ev_comp[k], st));
+        const int e0 = k == 0 ? 1 : i0;             // node plane 0 needs the last slab's cells
+        if (i1 > e0) {
+            if (M) {
+                ExpandStreamArgs ea{g, w.AM, dM, 0, e0, i1};
+                if (c->m_layout == ECSIM_M_14) k_expand_M_stream<14><<<(i1 - e0) * g.ny, XS_THREADS, XS_SMEM_BYTES, st>>>(ea);
+                else k_expand_M_stream<27><<<(i1 - e0) * g.ny, XS_THREADS, XS_SMEM_BYTES, st>>>(ea);
+                CK_LAUNCH();
+                c->launches++;
+            }
+            for (int s = 0; s < nsp && (rho || Jhat); ++s) {
+                ExpandJArgs ja{g, fa.sp[s].AJ, rho ? drho + (all_species_call ? s * nodes : 0) : nullptr,
+                               Jhat ? dJ + (all_species_call ? s * 3 * nodes : 0) : nullptr, 0, (long long)(e0 * plane), (long long)(i1 * plane)};
+                k_expand_rhoJ<<<(unsigned)(((size_t)(i1 - e0) * plane + 255) / 256), 256, 0, st>>>(ja);
+                CK_LAUNCH();
+                c->launches++;
+            }
+        }
+        CK(cudaEventRecord(c->ev_exp[k], st));
+        // ---- download ----
+        CK(cudaStreamWaitEvent(down, c->ev_comp[k], 0));
+        for (int s = 0; s < nsp; ++s) {
+            const size_t p0 = P[s][k], cnt = (size_t)P[s][k + 1] - p0, pn = (size_t)n[s];
+            if (!cnt) continue;
+            for (int a = 0; a < 6; ++a)
+                CK(cudaMemcpyAsync(hp[s * 7 + a] + p0, dpart + sp_off[s] + a * pn + p0, sizeof(double) * cnt, cudaMemcpyDeviceToHost, down));
+        }
+        CK(cudaStreamWaitEvent(down, c->ev_exp[k], 0));
+        if (M && i1 > e0)
+            CK(cudaMemcpyAsync(M + (size_t)e0 * plane * mper, dM + (size_t)e0 * plane * mper, sizeof(double) * (size_t)(i1 - e0) * plane * mper,
+                               cudaMemcpyDeviceToHost, down));
+    }
+    // node plane 0 (cells of the last and the first plane), then rho / Jhat in one piece
+    if (M) {
+        ExpandStreamArgs ea{g, w.AM, dM, 0, 0, 1};
+        if (c->m_layout == ECSIM_M_14) k_expand_M_stream<14><<<g.ny, XS_THREADS, XS_SMEM_BYTES, st>>>(ea);
+        else k_expand_M_stream<27><<<g.ny, XS_THREADS, XS_SMEM_BYTES, st>>>(ea);
+        CK_LAUNCH();
+        c->launches++;
+    }
+    for (int s = 0; s < nsp && (rho || Jhat); ++s) {
+        ExpandJArgs ja{g, fa.sp[s].AJ, rho ? drho + (all_species_call ? s * nodes : 0) : nullptr,
+                       Jhat ? dJ + (all_species_call ? s * 3 * nodes : 0) : nullptr, 0, 0, (long long)plane};
+        k_expand_rhoJ<<<(unsigned)((plane + 255) / 256), 256, 0, st>>>(ja);
+        CK_LAUNCH();
+        c->launches++;
+    }
+    uint32_t h_bad[ECSIM_MAX_SPECIES] = {};
+    CK(cudaMemcpyAsync(h_bad, bad, sizeof(uint32_t) * nsp, cudaMemcpyDeviceToHost, st));
+    if (M) CK(cudaMemcpyAsync(M, dM, sizeof(double) * plane * mper, cudaMemcpyDeviceToHost, st));
+    const int nout = all_species_call ? nsp : 1;
+    if (rho) CK(cudaMemcpyAsync(rho, drho, sizeof(double) * nodes * nout, cudaMemcpyDeviceToHost, st));
+    if (Jhat) CK(cudaMemcpyAsync(Jhat, dJ, sizeof(double) * 3 * nodes * nout, cudaMemcpyDeviceToHost, st));
+    CK(cudaEventRecord(c->ev_down, down));
+    CK(cudaStreamWaitEvent(st, c->ev_down, 0));
+    CK(cudaStreamSynchronize(st));
+    for (int s = 0; s < nsp; ++s)
+        if (h_bad[s]) {
+            // (bad and the stray counters share storage: a particle outside the slab its place in the arrays implies, or
+            // outside its cell's segment.)  The pushed particles of earlier slabs are already in the caller's arrays:
+            // there is no way back to the serial path.
+            snprintf(g_last_error, sizeof(g_last_error), "host step: species %d was declared cell-sorted but %u particle(s) "
+                     "are out of order; particle arrays are partially advanced", s, h_bad[s]);
+            return ECSIM_ERR_INVALID_ARG;
+        }
+    c->host_pipelined_calls++;
+    return ECSIM_OK;
+}
+
 // nsp species (slots 0..nsp-1 of the context) from host arrays; rho [nsp][nodes], Jhat [nsp][3][nodes], M shared.
 static int host_step_impl(ecsim_ctx* c, int nsp, const int64_t* n, const double* qom, int sorted,
                           double* const* hx, double* const* hy, double* const* hz, double* const* hu,
@@ -1250,6 +1461,17 @@ static int host_step_impl(ecsim_ctx* c, int nsp, const int64_t* n, const double*
             if (c->sp[s].state == ST_SEGMENTED && !c->sp[s].res.on) c->sp[s].state = ST_DECLARED;   // the tables lived in the re-carved buffer
     };
     auto body = [&]() -> int {
+        if (c->host_pipeline && sorted && accumulate == ECSIM_ACC_NONE && c->variant == ECSIM_VARIANT_FUSED) {
+            double* hp[ECSIM_MAX_SPECIES * 7];
+            for (int s = 0; s < nsp; ++s) {
+                double* a7[7] = {hx[s], hy[s], hz[s], hu[s], hv[s], hw[s], const_cast<double*>(hq[s])};
+                for (int a = 0; a < 7; ++a) hp[s * 7 + a] = a7[a];
+            }
+            const int prc = host_step_pipelined(c, nsp, n, qom, hp, E_theta, B, dt, theta, rho, Jhat, M, all_species_call,
+                                                dpart, dE, dB, drho, dJ, dM);
+            if (prc <= 0) return prc;          // done, or failed
+            // 1: not applicable (too small, an empty species, plane 0 not first): nothing was touched, go on serially
+        }
         double* d = dpart;
         for (int s = 0; s < nsp; ++s) {
             const size_t pn = (size_t)n[s];

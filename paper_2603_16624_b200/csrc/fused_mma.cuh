@@ -300,19 +300,33 @@ __device__ __forceinline__ int dest_coord(double x, double rd, int n)
 // need for its own particles (all it holds now) plus the arrivals so far stay inside the segment -- a bound that needs
 // no coordination with the warp that owns the cell.  Otherwise the particle goes to the species' overflow list and the
 // next call lays the species out afresh.
-__device__ __forceinline__ void relocate(const Geom& g, const SpeciesDev& sp, const PushedRegs& o, double q)
+struct Relocation { uint32_t d, a, room, s1; };
+
+// first half: the new cell and a ticket from its arrival counter.  (Requesting the ticket before phase 2 and using it
+// after -- to hide the atomic's latency -- was measured: no gain, 0.2-0.5 ms slower per step at configs[2]; the 14 extra
+// live registers cost more than the few stalled warps.)
+__device__ __forceinline__ Relocation relocate_begin(const Geom& g, const SpeciesDev& sp, const PushedRegs& o)
 {
     const int di = dest_coord(o.x, g.rdx, g.nx), dj = dest_coord(o.y, g.rdy, g.ny), dk = dest_coord(o.z, g.rdz, g.nz);
-    const uint32_t d = (uint32_t)((di * g.ny + dj) * g.nz + dk);
-    const uint32_t s0 = __ldg(sp.seg + d), s1 = __ldg(sp.seg + d + 1);
-    const uint32_t held = __ldg(sp.Fin + d) + __ldg(sp.Rin + d);
-    const uint32_t a = atomicAdd(sp.Rout + d, 1u);
-    if (held + a < s1 - s0) {
-        const uint32_t pos = s1 - 1u - a;
+    Relocation r;
+    r.d = (uint32_t)((di * g.ny + dj) * g.nz + dk);
+    const uint32_t s0 = __ldg(sp.seg + r.d);
+    r.s1 = __ldg(sp.seg + r.d + 1);
+    const uint32_t held = __ldg(sp.Fin + r.d) + __ldg(sp.Rin + r.d);
+    r.room = r.s1 - s0 > held ? r.s1 - s0 - held : 0u;
+    r.a = atomicAdd(sp.Rout + r.d, 1u);
+    return r;
+}
+
+// second half: the slot, or the overflow list
+__device__ __forceinline__ void relocate_end(const SpeciesDev& sp, const Relocation& r, const PushedRegs& o, double q)
+{
+    if (r.a < r.room) {
+        const uint32_t pos = r.s1 - 1u - r.a;
         sp.ox[pos] = o.x; sp.oy[pos] = o.y; sp.oz[pos] = o.z;
         sp.ou[pos] = o.u; sp.ov[pos] = o.v; sp.ow[pos] = o.w; sp.oq[pos] = q;
     } else {
-        atomicSub(sp.Rout + d, 1u);          // slots >= the bound are never handed out: the counter ends at min(arrivals, room)
+        atomicSub(sp.Rout + r.d, 1u);        // slots >= the bound are never handed out: the counter ends at min(arrivals, room)
         const uint32_t k = atomicAdd(sp.ovf_count, 1u);
         if (k < sp.ovf_cap) {
             double* v = sp.ovf + k;
@@ -320,6 +334,12 @@ __device__ __forceinline__ void relocate(const Geom& g, const SpeciesDev& sp, co
             v[0] = o.x; v[m] = o.y; v[2 * m] = o.z; v[3 * m] = o.u; v[4 * m] = o.v; v[5 * m] = o.w; v[6 * m] = q;
         }
     }
+}
+
+__device__ __forceinline__ void relocate(const Geom& g, const SpeciesDev& sp, const PushedRegs& o, double q)
+{
+    const Relocation r = relocate_begin(g, sp, o);
+    relocate_end(sp, r, o, q);
 }
 
 // REGS: register cap.  Measured on config 2 (whole grid, ms): 12 warps x 168 regs 11.89, 12 x 144 12.23, 16 x 128

@@ -45,6 +45,35 @@ k_cell_hist(Geom g, uint32_t n, const double* __restrict__ x, const double* __re
     }
 }
 
+// Histogram of the particles [p0, p1) of a cell-sorted species that must all lie in the cells [c0, c1) (one x-slab of the
+// pipelined host step): particles outside the range are counted in *bad instead (the caller then falls back).
+__global__ void __launch_bounds__(256)
+k_cell_hist_range(Geom g, uint32_t p0, uint32_t p1, const double* __restrict__ x, const double* __restrict__ y,
+                  const double* __restrict__ z, uint32_t* __restrict__ count, uint32_t c0, uint32_t c1,
+                  uint32_t* __restrict__ bad)
+{
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    const size_t n = (size_t)(p1 - p0), n_round = (n + 31) & ~(size_t)31;
+    for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < n_round; t += stride) {
+        const bool active = t < n;
+        int c = -1;
+        if (active) {
+            const size_t p = p0 + t;
+            c = cell_of(g, x[p], y[p], z[p]);
+            if ((uint32_t)c < c0 || (uint32_t)c >= c1) { atomicAdd(bad, 1u); c = -1; }
+        }
+        const unsigned peers = __match_any_sync(0xffffffffu, c);
+        if (c >= 0 && (int)lane_id() == __ffs(peers) - 1) atomicAdd(&count[c], (uint32_t)__popc(peers));
+    }
+}
+
+__global__ void __launch_bounds__(256)
+k_add_u32(uint32_t* __restrict__ a, uint32_t m, uint32_t v)
+{
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < m) a[i] += v;
+}
+
 // Cell id only (ecsim_cell_index).
 __global__ void __launch_bounds__(256)
 k_cell_index(Geom g, uint32_t n, const double* __restrict__ x, const double* __restrict__ y,

@@ -392,3 +392,59 @@ def test_host_buffer_all_species_step_matches_oracle():
     assert_moments_close(None, None, M, total, "host all")
     # the single-species host call still works on the same context afterwards
     ctx.close()
+
+
+@pytest.mark.parametrize("idx,scale", [(0, None), (3, (6, 48, 6)), (2, (9, 4, 5))], ids=["cfg0", "cfg3", "cfg2_odd"])
+def test_pipelined_host_step_matches_oracle(idx, scale):
+    """The host-buffer entry as a three-stream pipeline over slabs of x-planes (upload | compute | download); forced on a
+    small input with ecsim_set_host_pipeline(2).  Same parity as the serial path; both M layouts."""
+    cfg = wl.config(idx, scale)
+    E, B = wl.gen_fields(cfg)
+    parts = [wl.gen_species(cfg, s, shuffle=False) for s in range(2)]
+    for layout in (pk.M_27, pk.M_14):
+        parts_np = [to_numpy(p) for p in parts]
+        host = [{k: p[k].clone().pin_memory() for k in PKEYS} for p in parts]
+        ctx = pk.Ecsim(*grid_of(cfg), 2)
+        ctx.set_workspace_host_all(max(p["n"] for p in parts), sum(p["n"] for p in parts))
+        ctx.set_host_pipeline(2)
+        ctx.set_m_layout(layout)
+        rho = torch.full((2, cfg.nodes), float("nan"), dtype=torch.float64).pin_memory()
+        J = torch.full((2, 3, cfg.nodes), float("nan"), dtype=torch.float64).pin_memory()
+        M = torch.full((cfg.nodes, 27 if layout == pk.M_27 else 14, 3, 3), float("nan"), dtype=torch.float64).pin_memory()
+        ctx.push_and_moments_host_all([sp.qom for sp in cfg.species], True, host, E.contiguous(), B.contiguous(), cfg.dt,
+                                      cfg.theta, rho, J, M)
+        assert ctx.host_pipelined_count() == 1
+        (total, per_species), = oracle_run(cfg, parts_np, E, B)
+        for s in range(2):
+            assert_particles_close(host[s], parts_np[s], cfg, f"pipelined host step, species {s}")
+            assert_moments_close(rho[s], J[s], None, per_species[s], f"pipelined host step, species {s}")
+        if layout == pk.M_27:
+            assert_moments_close(None, None, M, total, "pipelined host step")
+        else:
+            Mn = M.numpy()
+            assert np.all(np.isfinite(Mn))
+            assert np.all(np.abs(Mn - total.M[:, 13:]) <= 1e-10 * total.M_abs[:, 13:])
+        ctx.close()
+
+
+def test_pipelined_host_step_rejects_unsorted_input_declared_sorted():
+    cfg = wl.config(0)
+    E, B = wl.gen_fields(cfg)
+    part = wl.gen_species(cfg, 0, shuffle=True)
+    host = {k: part[k].clone().pin_memory() for k in PKEYS}
+    ctx = pk.Ecsim(*grid_of(cfg), 1)
+    ctx.set_workspace(part["n"], host_step=True)
+    ctx.set_host_pipeline(2)
+    rho = torch.empty(cfg.nodes, dtype=torch.float64).pin_memory()
+    J = torch.empty(3, cfg.nodes, dtype=torch.float64).pin_memory()
+    M = torch.empty(cfg.nodes, 27, 3, 3, dtype=torch.float64).pin_memory()
+    with pytest.raises(pk.EcsimError, match="out of order|invalid"):
+        ctx.push_and_moments_host(cfg.species[0].qom, True, host, E.contiguous(), B.contiguous(), cfg.dt, cfg.theta, rho, J, M)
+    # declared unsorted: the serial path sorts, and is right
+    pn = to_numpy(part)
+    host = {k: part[k].clone().pin_memory() for k in PKEYS}
+    ctx.push_and_moments_host(cfg.species[0].qom, False, host, E.contiguous(), B.contiguous(), cfg.dt, cfg.theta, rho, J, M)
+    mom = oracle.Moments(cfg.nodes)
+    oracle.step(grid_of(cfg), cfg.species[0].qom, cfg.dt, pn, E.numpy(), B.numpy(), mom)
+    assert_moments_close(rho, J, M, mom, "host step, unsorted")
+    ctx.close()
