@@ -70,7 +70,7 @@ def parse_args():
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (default 2, the headline)")
     ap.add_argument("--scale", default=None, help="nx,ny,nz override of the grid (tests / quick runs)")
     ap.add_argument("--variant", default="fused", choices=["fused", "atomic"])
-    ap.add_argument("--fused-warps", type=int, default=-1, help="8/12/16 warps of the unified kernel, 0 = warp-specialised")
+    ap.add_argument("--fused-warps", type=int, default=-1, help="8 / 12 / 16 warps per CTA of the fused kernel (library default 12)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -270,7 +270,7 @@ def run_product(args):
     ctx = pk.Ecsim(*grid_of(cfg), nsp)
     ctx.set_workspace(max(n_s))
     ctx.set_variant(pk.VARIANT_FUSED if args.variant == "fused" else pk.VARIANT_ATOMIC)
-    if args.fused_warps >= 0:
+    if args.fused_warps > 0:
         ctx.set_fused_warps(args.fused_warps)
     ctx.enable_timing(True)
     rho = torch.empty(nsp, cfg.nodes, dtype=torch.float64, device=dev)

@@ -13,7 +13,6 @@
 #include "sort.cuh"
 #include "atomic_path.cuh"
 #include "fused_mma.cuh"
-#include "fused_ws.cuh"
 #include "expand.cuh"
 #include "expand_tma.cuh"
 #include "resident.cuh"
@@ -762,7 +761,7 @@ extern "C" int ecsim_set_resort_fraction(ecsim_ctx* c, double fraction)
 
 extern "C" int ecsim_set_fused_warps(ecsim_ctx* c, int warps)
 {
-    if (!c || (warps != 0 && warps != 8 && warps != 12 && warps != 16 && warps != 13 && warps != 17)) return ECSIM_ERR_INVALID_ARG;
+    if (!c || (warps != 8 && warps != 12 && warps != 16)) return ECSIM_ERR_INVALID_ARG;
     c->fused_warps = warps;
     return ECSIM_OK;
 }
@@ -812,40 +811,23 @@ extern "C" int64_t ecsim_leaver_count(ecsim_ctx* c)
     return total;
 }
 
-template <int NW, int REGS, int MODE, int LAYOUT, bool EARLY = false>
+template <int NW, int REGS, int MODE, int LAYOUT>
 static cudaError_t launch_fused(const ecsim_ctx* c, const FusedArgs& fa)
 {
     const size_t smem = (size_t)NW * (MODE == MODE_PUSH ? FLD_DOUBLES : WARP_SMEM_DOUBLES) * sizeof(double);
     // per launch, not per process: a second device of the same process needs its own opt-in
-    cudaError_t e = cudaFuncSetAttribute(k_fused_push_moments<NW, REGS, MODE, LAYOUT, EARLY>,
+    cudaError_t e = cudaFuncSetAttribute(k_fused_push_moments<NW, REGS, MODE, LAYOUT>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const size_t cells = (size_t)(fa.c_end - fa.c_begin);
     size_t grid = (cells + NW - 1) / NW;
     if (grid > (size_t)c->sm_count) grid = (size_t)c->sm_count;
-    k_fused_push_moments<NW, REGS, MODE, LAYOUT, EARLY><<<(int)grid, NW * 32, smem, c->stream>>>(fa);
-    return cudaGetLastError();
-}
-
-template <int MODE, int LAYOUT>
-static cudaError_t launch_ws(const ecsim_ctx* c, const FusedArgs& fa)
-{
-    cudaError_t e = cudaFuncSetAttribute(k_fused_ws<MODE, LAYOUT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)WS_SMEM_BYTES);
-    if (e != cudaSuccess) return e;
-    const size_t cells = (size_t)(fa.c_end - fa.c_begin);
-    size_t grid = (cells + WS_PAIRS - 1) / WS_PAIRS;
-    if (grid > (size_t)c->sm_count) grid = (size_t)c->sm_count;
-    k_fused_ws<MODE, LAYOUT><<<(int)grid, WS_WARPS * 32, WS_SMEM_BYTES, c->stream>>>(fa);
+    k_fused_push_moments<NW, REGS, MODE, LAYOUT><<<(int)grid, NW * 32, smem, c->stream>>>(fa);
     return cudaGetLastError();
 }
 
 static cudaError_t launch_fused_any(const ecsim_ctx* c, const FusedArgs& fa, int mode, bool gapped)
 {
-    if (c->fused_warps == 0 && (mode == MODE_FUSED || mode == MODE_MOMENTS)) {
-        if (mode == MODE_FUSED)
-            return gapped ? launch_ws<MODE_FUSED, LAYOUT_GAPPED>(c, fa) : launch_ws<MODE_FUSED, LAYOUT_DENSE>(c, fa);
-        return gapped ? launch_ws<MODE_MOMENTS, LAYOUT_GAPPED>(c, fa) : launch_ws<MODE_MOMENTS, LAYOUT_DENSE>(c, fa);
-    }
     if (mode == MODE_DIAG)
         return gapped ? launch_fused<16, 128, MODE_DIAG, LAYOUT_GAPPED>(c, fa) : launch_fused<16, 128, MODE_DIAG, LAYOUT_DENSE>(c, fa);
     if (mode == MODE_PUSH)
@@ -853,8 +835,6 @@ static cudaError_t launch_fused_any(const ecsim_ctx* c, const FusedArgs& fa, int
     if (mode == MODE_MOMENTS)
         return gapped ? launch_fused<12, 168, MODE_MOMENTS, LAYOUT_GAPPED>(c, fa) : launch_fused<12, 168, MODE_MOMENTS, LAYOUT_DENSE>(c, fa);
     if (gapped) return launch_fused<12, 168, MODE_FUSED, LAYOUT_GAPPED>(c, fa);
-    if (c->fused_warps == 13) return launch_fused<12, 168, MODE_FUSED, LAYOUT_DENSE, true>(c, fa);   // experiment: early fetch
-    if (c->fused_warps == 17) return launch_fused<16, 128, MODE_FUSED, LAYOUT_DENSE, true>(c, fa);
     if (c->fused_warps == 8) return launch_fused<8, 224, MODE_FUSED, LAYOUT_DENSE>(c, fa);
     if (c->fused_warps == 16) return launch_fused<16, 128, MODE_FUSED, LAYOUT_DENSE>(c, fa);
     return launch_fused<12, 168, MODE_FUSED, LAYOUT_DENSE>(c, fa);

@@ -344,7 +344,7 @@ __device__ __forceinline__ void relocate(const Geom& g, const SpeciesDev& sp, co
 
 // REGS: register cap.  Measured on config 2 (whole grid, ms): 12 warps x 168 regs 11.89, 12 x 144 12.23, 16 x 128
 // 12.15, 12 x 128 12.88, 8 x 200 13.63; warp counts that are not a multiple of the 4 schedulers lose (14 x 128 13.58).
-template <int NW, int REGS, int MODE, int LAYOUT, bool EARLY = false>
+template <int NW, int REGS, int MODE, int LAYOUT>
 __global__ void __maxnreg__(REGS)
 k_fused_push_moments(const __grid_constant__ FusedArgs a)
 {
@@ -513,12 +513,6 @@ k_fused_push_moments(const __grid_constant__ FusedArgs a)
                 }
             }
 
-            // EARLY: the next batch's loads are requested before this batch's phase 1 (more time to land, 14 more live registers)
-            if (EARLY) {
-                if (in_state == 1 || in_state == 2) fetch();
-                if (in_state != 1 && has_next) { load_fields(ni, nj, nk, f0, f1); fld_ready = true; }
-            }
-
             // ---- phase 1: lane = particle ----
             PushedRegs o;
             const bool active = lane < nb;
@@ -542,11 +536,10 @@ k_fused_push_moments(const __grid_constant__ FusedArgs a)
                     my_leavers += o.stays ? 0u : 1u;
                 }
             }
-            // global loads of the next batch fly during phase 2
-            if (!EARLY) {
-                if (in_state == 1 || in_state == 2) fetch();
-                if (in_state != 1 && has_next) { load_fields(ni, nj, nk, f0, f1); fld_ready = true; }
-            }
+            // global loads of the next batch fly during phase 2 (requesting them before phase 1 was measured: 11.90 vs
+            // 11.65 ms, the 14 extra live registers cost more than the longer flight time gains)
+            if (in_state == 1 || in_state == 2) fetch();
+            if (in_state != 1 && has_next) { load_fields(ni, nj, nk, f0, f1); fld_ready = true; }
             if (!GAPPED) {
                 const unsigned smask = __ballot_sync(0xffffffffu, active && !inside);
                 if (smask) {

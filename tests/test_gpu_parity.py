@@ -71,10 +71,7 @@ def test_cell_index_and_counting_sort_are_bit_exact(case):
 
 # ------------------------------------------------------------------ the hot path, all five configs
 
-WS = "fused_ws"      # the warp-specialised form of the fused kernel (csrc/fused_ws.cuh): ecsim_set_fused_warps(0)
-
-
-@pytest.mark.parametrize("variant", [pk.VARIANT_FUSED, WS, pk.VARIANT_ATOMIC], ids=["fused", "fused_ws", "atomic"])
+@pytest.mark.parametrize("variant", [pk.VARIANT_FUSED, pk.VARIANT_ATOMIC], ids=["fused", "atomic"])
 @pytest.mark.parametrize("case", list(CASES))
 def test_push_and_moments_match_oracle(case, variant):
     idx, scale = CASES[case]
@@ -85,12 +82,7 @@ def test_push_and_moments_match_oracle(case, variant):
     parts_np = [to_numpy(p) for p in parts]
     parts_cuda = [to_cuda(p) for p in parts]
     n_max = max(p["n"] for p in parts)
-    ws = variant == WS
-    if ws:
-        variant = pk.VARIANT_FUSED
     ctx = make_ctx(cfg, n_max, variant)
-    if ws:
-        ctx.set_fused_warps(0)
     perms = None
     if cfg.shuffled and variant == pk.VARIANT_FUSED:
         # config 4: particles arrive in random order; sort explicitly to learn the permutation
