@@ -80,7 +80,7 @@ struct Workspace {
     int32_t* cell = nullptr;         // [n_max]
     uint32_t* rank = nullptr;        // [n_max]
     uint32_t* perm = nullptr;        // [n_max]
-    double* spare = nullptr;         // [n_max]
+    double* spare = nullptr;         // [7][n_max]: the seven arrays of a species on their way through a sort
     uint32_t* tile_hist = nullptr;   // [buckets][tiles] of the two-step move of a random-order sort
     uint32_t* tile_scan = nullptr;   // its exclusive scan (+1)
     uint32_t* tile_sums = nullptr;   // block sums of that scan
@@ -149,7 +149,7 @@ static size_t carve(const ecsim_ctx* c, int64_t n_max, void* base, Workspace* ou
     w.cell = k.take<int32_t>(n);
     w.rank = k.take<uint32_t>(n);
     w.perm = k.take<uint32_t>(n);
-    w.spare = k.take<double>(n);
+    w.spare = k.take<double>(7 * n);
     {
         const size_t m = (size_t)SORT_MAX_BUCKETS * (n / SORT_TILE + 1);
         w.tile_hist = k.take<uint32_t>(m);
@@ -289,7 +289,7 @@ extern "C" int ecsim_set_workspace(ecsim_ctx* c, void* dev_ptr, size_t bytes)
     // n_max = the largest particle count the buffer can serve
     const size_t fixed = carve(c, 0, nullptr, nullptr);
     if (bytes < fixed) return ECSIM_ERR_WORKSPACE;
-    const size_t per_particle = sizeof(int32_t) + 2 * sizeof(uint32_t) + sizeof(double) +
+    const size_t per_particle = sizeof(int32_t) + 2 * sizeof(uint32_t) + 7 * sizeof(double) +
                                 (size_t)c->n_species * sizeof(uint32_t);
     // carve() is monotone in n: bisect for the largest n that fits (the per-array 256-byte rounding
     // makes a closed form off by a few particles either way)
@@ -467,30 +467,34 @@ extern "C" int ecsim_sort_particles(ecsim_ctx* c, int s, int32_t* cell_count_out
         const uint32_t n = (uint32_t)sp.n;
         const int grid = grid_for(c, (size_t)sp.n, 256, 16);
         double* arrays[7] = {sp.x, sp.y, sp.z, sp.u, sp.v, sp.w, sp.q};
+        const size_t nmax = (size_t)w.n_max;
         if (sp.nearly_sorted) {
-            // a re-sort after pushes: perm is close to the identity, the gather reads almost sequentially
+            // a re-sort after pushes: perm is close to the identity, the gather reads almost sequentially; the seven
+            // arrays in one launch (the permutation is read once), then back into the caller's arrays
             k_build_perm<<<grid, 256, 0, c->stream>>>(n, w.cell, w.rank, start, w.perm);
             CK_LAUNCH();
-            c->launches++;
+            Move7 mv;
+            for (int a = 0; a < 7; ++a) { mv.src[a] = arrays[a]; mv.dst[a] = w.spare + a * nmax; }
+            k_gather7<<<grid, 256, 0, c->stream>>>(n, w.perm, mv);
+            CK_LAUNCH();
+            c->launches += 2;
             for (int a = 0; a < 7; ++a) {
-                k_gather_f64<<<grid, 256, 0, c->stream>>>(n, w.perm, arrays[a], w.spare);
-                CK_LAUNCH();
-                CK(cudaMemcpyAsync(arrays[a], w.spare, sizeof(double) * (size_t)n, cudaMemcpyDeviceToDevice, c->stream));
-                c->launches += 2;
+                CK(cudaMemcpyAsync(arrays[a], w.spare + a * nmax, sizeof(double) * (size_t)n, cudaMemcpyDeviceToDevice, c->stream));
+                c->launches++;
             }
             if (perm_out)
                 CK(cudaMemcpyAsync(perm_out, w.perm, sizeof(uint32_t) * (size_t)n, cudaMemcpyDeviceToDevice, c->stream));
         } else {
-            // arbitrary order: the bucketed two-step move of sort.cuh
-            CK(cudaFuncSetAttribute(k_stage_to_slots, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SORT_STAGE_SMEM));
+            // arbitrary order: the bucketed two-step move of sort.cuh, seven arrays per launch
+            CK(cudaFuncSetAttribute(k_stage7_to_slots, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SORT_STAGE_SMEM));
             int shift = 13;
             while ((((n - 1) >> shift) + 1) > (uint32_t)SORT_MAX_BUCKETS) ++shift;
             const uint32_t nbk = ((n - 1) >> shift) + 1;
             const uint32_t tiles = (n + SORT_TILE - 1) / SORT_TILE;
             const uint32_t m = nbk * tiles;
             uint32_t* dest = w.rank;                                   // rank -> dest in place
-            uint32_t* slot = reinterpret_cast<uint32_t*>(w.cell);      // the cell ids are not needed after that
-            uint32_t* perm2 = w.perm;
+            uint32_t* tmpdest = w.perm;
+            uint32_t* tmpidx = perm_out ? reinterpret_cast<uint32_t*>(w.cell) : nullptr;   // the cell ids are not needed after dest
             k_dest_and_tile_hist<<<tiles, 256, 0, c->stream>>>(n, w.cell, dest, start, shift, tiles, w.tile_hist);
             CK_LAUNCH();
             const uint32_t sb = (m + SCAN_BLOCK - 1) / SCAN_BLOCK;
@@ -500,22 +504,21 @@ extern "C" int ecsim_sort_particles(ecsim_ctx* c, int s, int32_t* cell_count_out
             CK_LAUNCH();
             k_scan_add<<<sb, SCAN_BLOCK, 0, c->stream>>>(w.tile_scan, w.tile_sums, m);
             CK_LAUNCH();
-            k_assign_slots<<<tiles, 256, 0, c->stream>>>(n, dest, w.tile_scan, shift, tiles, slot, perm2);
-            CK_LAUNCH();
-            c->launches += 5;
+            Sort7 s7;
+            Move7 mv;
             for (int a = 0; a < 7; ++a) {
-                k_stage_to_slots<<<tiles, SORT_STAGE_THREADS, SORT_STAGE_SMEM, c->stream>>>(
-                    n, dest, slot, w.tile_hist, w.tile_scan, shift, tiles, arrays[a], w.spare);
-                CK_LAUNCH();
-                k_gather_f64<<<grid, 256, 0, c->stream>>>(n, perm2, w.spare, arrays[a]);
-                CK_LAUNCH();
-                c->launches += 2;
+                s7.in[a] = arrays[a]; s7.tmp[a] = w.spare + a * nmax;
+                mv.src[a] = w.spare + a * nmax; mv.dst[a] = arrays[a];
             }
-            if (perm_out) {
-                k_perm_from_dest<<<grid, 256, 0, c->stream>>>(n, dest, perm_out);
-                CK_LAUNCH();
-                c->launches++;
-            }
+            k_stage7_to_slots<<<tiles, SORT_STAGE_THREADS, SORT_STAGE_SMEM, c->stream>>>(n, dest, w.tile_hist, w.tile_scan, shift,
+                                                                                      tiles, s7, tmpdest, tmpidx);
+            CK_LAUNCH();
+            uint32_t* perm2 = w.stray_list + (size_t)s * (size_t)w.n_max;      // (the stray lists are idle during a sort)
+            k_invert_slots<<<grid, 256, 0, c->stream>>>(n, tmpdest, perm2, tmpidx, perm_out);
+            CK_LAUNCH();
+            k_gather7<<<grid, 256, 0, c->stream>>>(n, perm2, mv);
+            CK_LAUNCH();
+            c->launches += 7;
         }
     }
     if (cell_count_out) {

@@ -4,7 +4,8 @@
 //   k_cell_hist   cell id per particle (+ its rank inside the cell) and the per-cell histogram
 //   k_scan_*      exclusive scan of the histogram -> start[cells+1]
 //   k_build_perm  perm[start[cell] + rank] = old index
-//   k_gather_f64  out[new] = in[perm[new]]   (one SoA array at a time)
+//   k_gather7     out[new] = in[perm[new]] for the seven SoA arrays (re-sort of a nearly sorted species)
+//   k_stage7_to_slots / k_scatter7  the two-step move of a species in arbitrary order
 //
 // Integer work only; results (cell ids, counts) are bit-exact functions of the stored positions.
 #pragma once
@@ -162,15 +163,6 @@ k_build_perm(uint32_t n, const int32_t* __restrict__ cell, const uint32_t* __res
 }
 
 __global__ void __launch_bounds__(256)
-k_gather_f64(uint32_t n, const uint32_t* __restrict__ perm, const double* __restrict__ in,
-             double* __restrict__ out)
-{
-    const size_t stride = (size_t)gridDim.x * blockDim.x;
-    for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += stride)
-        out[p] = in[perm[p]];
-}
-
-__global__ void __launch_bounds__(256)
 k_copy_u32_to_i32(uint32_t m, const uint32_t* __restrict__ in, int32_t* __restrict__ out)
 {
     const size_t stride = (size_t)gridDim.x * blockDim.x;
@@ -185,18 +177,21 @@ k_copy_u32_to_i32(uint32_t m, const uint32_t* __restrict__ in, int32_t* __restri
 // two steps that are both local.  dest[p] = start[cell[p]] + rank[p] is the final place of particle p;
 // places are cut into <= SORT_MAX_BUCKETS buckets of 2^shift consecutive places (every bucket is full,
 // dest being a permutation).
-//   step A, k_stage_to_slots: a tile of SORT_TILE particles per CTA.  slot[p] = (places of p's bucket taken by
-//          earlier tiles) + (p's arrival rank in the tile).  The tile is ordered by bucket in shared memory and
-//          written to tmp[] in runs of ~SORT_TILE/buckets consecutive elements: coalesced.
-//   step B, k_gather_f64 with perm2[dest[p]] = slot[p]: out[d] = tmp[perm2[d]], a gather whose sources lie
-//          inside one bucket's window of tmp (<= 1 MB): L2 hits; the writes are coalesced.
-// slot and perm2 are computed once and serve all seven arrays; tmp is the one spare array and `out` is the
-// caller's own array, so nothing is copied back.  (A species that is re-sorted after a push is nearly
-// sorted: there the direct gather of ecsim_sort_particles reads almost sequentially and stays.)
+//   step A, k_stage7_to_slots: a tile of SORT_TILE particles per CTA.  A particle's slot = (places of its bucket taken
+//          by earlier tiles, from the scanned per-(bucket, tile) histogram) + (its arrival rank in the tile, a shared-
+//          memory atomic).  The tile is ordered by bucket in shared memory and written to tmp[] in runs of
+//          ~SORT_TILE/buckets consecutive elements: coalesced.  ALL SEVEN arrays go through one launch -- the slot
+//          bookkeeping is computed once, kept in registers, and the final place travels with the particle (tmpdest).
+//   step B, k_invert_slots + k_gather7: perm2 = tmpdest^-1, then out[d] = tmp[perm2[d]] for the seven arrays: a gather
+//          whose sources lie inside the windows of the ~9 buckets in flight (grid-stride; 2^shift places x 7 arrays x 8 B
+//          = 3.5 MB each): L2 hits; the writes are coalesced.
+// Round 1 moved one array per launch pair (14 launches, the bookkeeping re-read 7 times, a separate slot-assignment
+// pass with a random 4-byte scatter): 4.35 ms per 33.5 M particles.  tmp = seven spare arrays of the workspace.
 constexpr int SORT_TILE = 8192;
 constexpr int SORT_MAX_BUCKETS = 512;
 constexpr int SORT_STAGE_THREADS = 512;
-constexpr size_t SORT_STAGE_SMEM = (size_t)SORT_TILE * (sizeof(double) + sizeof(uint32_t)) + 2 * SORT_MAX_BUCKETS * sizeof(uint32_t);
+constexpr int SORT_PER_THREAD = SORT_TILE / SORT_STAGE_THREADS;
+constexpr size_t SORT_STAGE_SMEM = (size_t)SORT_TILE * (sizeof(double) + sizeof(uint32_t)) + 3 * SORT_MAX_BUCKETS * sizeof(uint32_t);
 
 // dest (in place of rank) and the per-(bucket, tile) histogram H[b * tiles + tile]
 __global__ void __launch_bounds__(256)
@@ -220,38 +215,20 @@ k_dest_and_tile_hist(uint32_t n, const int32_t* __restrict__ cell, uint32_t* __r
     for (uint32_t b = threadIdx.x; b < nb; b += blockDim.x) H[(size_t)b * tiles + blockIdx.x] = cnt[b];
 }
 
-// slot[p] (over the cell array's storage) and perm2[dest[p]] = slot[p]; Hs = exclusive scan of H
-__global__ void __launch_bounds__(256)
-k_assign_slots(uint32_t n, const uint32_t* __restrict__ dest, const uint32_t* __restrict__ Hs, int shift,
-               uint32_t tiles, uint32_t* __restrict__ slot, uint32_t* __restrict__ perm2)
-{
-    __shared__ uint32_t base[SORT_MAX_BUCKETS];
-    const uint32_t nb = ((n - 1) >> shift) + 1;
-    for (uint32_t b = threadIdx.x; b < nb; b += blockDim.x) base[b] = Hs[(size_t)b * tiles + blockIdx.x];
-    __syncthreads();
-    const size_t p0 = (size_t)blockIdx.x * SORT_TILE;
-    for (int e = threadIdx.x; e < SORT_TILE; e += blockDim.x) {
-        const size_t p = p0 + e;
-        if (p < n) {
-            const uint32_t d = dest[p];
-            const uint32_t s = atomicAdd(&base[d >> shift], 1u);
-            slot[p] = s;
-            perm2[d] = s;
-        }
-    }
-}
+struct Sort7 { const double* in[7]; double* tmp[7]; };
 
-// step A for one array: tmp[slot[p]] = in[p], the tile ordered by bucket in shared memory first
+// step A for the seven arrays of one tile.  H: per-(bucket, tile) histogram, Hs: its exclusive scan.
 __global__ void __launch_bounds__(SORT_STAGE_THREADS)
-k_stage_to_slots(uint32_t n, const uint32_t* __restrict__ dest, const uint32_t* __restrict__ slot,
-                 const uint32_t* __restrict__ H, const uint32_t* __restrict__ Hs, int shift, uint32_t tiles,
-                 const double* __restrict__ in, double* __restrict__ tmp)
+k_stage7_to_slots(uint32_t n, const uint32_t* __restrict__ dest, const uint32_t* __restrict__ H,
+                  const uint32_t* __restrict__ Hs, int shift, uint32_t tiles, Sort7 a, uint32_t* __restrict__ tmpdest,
+                  uint32_t* __restrict__ tmpidx /* or null */)
 {
     extern __shared__ __align__(16) unsigned char stage_smem[];
     double* vals = reinterpret_cast<double*>(stage_smem);
-    uint32_t* dsts = reinterpret_cast<uint32_t*>(vals + SORT_TILE);
+    uint32_t* dsts = reinterpret_cast<uint32_t*>(vals + SORT_TILE);   // slot of the element at tile position lp
     uint32_t* base = dsts + SORT_TILE;          // first slot of this tile's share of bucket b
     uint32_t* toff = base + SORT_MAX_BUCKETS;   // where bucket b starts in the tile's bucket order
+    uint32_t* cnt = toff + SORT_MAX_BUCKETS;    // arrivals so far
     __shared__ uint32_t total;
     const uint32_t nb = ((n - 1) >> shift) + 1;
     const uint32_t b = threadIdx.x;
@@ -259,18 +236,76 @@ k_stage_to_slots(uint32_t n, const uint32_t* __restrict__ dest, const uint32_t* 
     const uint32_t ex = block_exclusive_scan(c, &total);
     toff[b] = ex;
     base[b] = b < nb ? Hs[(size_t)b * tiles + blockIdx.x] : 0u;
+    cnt[b] = 0u;
     __syncthreads();
     const size_t p0 = (size_t)blockIdx.x * SORT_TILE;
     const uint32_t tile_n = (uint32_t)min((size_t)SORT_TILE, (size_t)n - p0);
-    for (uint32_t e = threadIdx.x; e < tile_n; e += SORT_STAGE_THREADS) {
-        const size_t p = p0 + e;
-        const uint32_t s = slot[p], bk = dest[p] >> shift;
-        const uint32_t lp = s - base[bk] + toff[bk];
-        vals[lp] = in[p];
-        dsts[lp] = s;
+    uint32_t lp[SORT_PER_THREAD];               // this thread's elements: their positions in the tile's bucket order
+    uint32_t* dvals = reinterpret_cast<uint32_t*>(vals);
+#pragma unroll
+    for (int j = 0; j < SORT_PER_THREAD; ++j) {
+        const uint32_t e = threadIdx.x + j * SORT_STAGE_THREADS;
+        lp[j] = 0xffffffffu;
+        if (e < tile_n) {
+            const uint32_t d = dest[p0 + e], bk = d >> shift;
+            const uint32_t r = atomicAdd(&cnt[bk], 1u);
+            lp[j] = toff[bk] + r;
+            dsts[lp[j]] = base[bk] + r;
+            dvals[lp[j]] = d;
+        }
     }
     __syncthreads();
-    for (uint32_t t = threadIdx.x; t < tile_n; t += SORT_STAGE_THREADS) tmp[dsts[t]] = vals[t];
+    for (uint32_t t = threadIdx.x; t < tile_n; t += SORT_STAGE_THREADS) tmpdest[dsts[t]] = dvals[t];
+    __syncthreads();
+    if (tmpidx) {
+#pragma unroll
+        for (int j = 0; j < SORT_PER_THREAD; ++j)
+            if (lp[j] != 0xffffffffu) dvals[lp[j]] = (uint32_t)(p0 + threadIdx.x + j * SORT_STAGE_THREADS);
+        __syncthreads();
+        for (uint32_t t = threadIdx.x; t < tile_n; t += SORT_STAGE_THREADS) tmpidx[dsts[t]] = dvals[t];
+        __syncthreads();
+    }
+#pragma unroll 1
+    for (int k = 0; k < 7; ++k) {
+        const double* __restrict__ in = a.in[k];
+        double* __restrict__ tmp = a.tmp[k];
+#pragma unroll
+        for (int j = 0; j < SORT_PER_THREAD; ++j)
+            if (lp[j] != 0xffffffffu) vals[lp[j]] = in[p0 + threadIdx.x + j * SORT_STAGE_THREADS];
+        __syncthreads();
+        for (uint32_t t = threadIdx.x; t < tile_n; t += SORT_STAGE_THREADS) tmp[dsts[t]] = vals[t];
+        __syncthreads();
+    }
+}
+
+struct Move7 { const double* src[7]; double* dst[7]; };
+
+// step B, first half: the inverse of tmpdest, perm2[tmpdest[t]] = t (a 4-byte scatter that stays inside the bucket's
+// window: L2), and the permutation for the caller if asked.  (Scattering the seven payload arrays the same way was
+// measured: 5.5 ms per 33.5 M particles, every 8-byte store a read-modify-write of its DRAM sector; the gather below
+// reads at random from the L2-resident window instead and writes whole sectors.)
+__global__ void __launch_bounds__(256)
+k_invert_slots(uint32_t n, const uint32_t* __restrict__ tmpdest, uint32_t* __restrict__ perm2,
+               const uint32_t* __restrict__ tmpidx, uint32_t* __restrict__ perm_out)
+{
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += stride) {
+        const uint32_t d = tmpdest[t];
+        perm2[d] = (uint32_t)t;
+        if (perm_out) perm_out[d] = tmpidx[t];
+    }
+}
+
+// re-sort of a nearly sorted species: dst[new] = src[perm[new]], seven arrays, the permutation read once
+__global__ void __launch_bounds__(256)
+k_gather7(uint32_t n, const uint32_t* __restrict__ perm, Move7 a)
+{
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += stride) {
+        const uint32_t q = perm[p];
+#pragma unroll
+        for (int k = 0; k < 7; ++k) a.dst[k][p] = a.src[k][q];
+    }
 }
 
 // fixPosition on stored particles (L123): pin the masked coordinates of n slots (set-up of a reduced-dimension run)
@@ -292,12 +327,4 @@ k_iota_u32(uint32_t n, uint32_t* __restrict__ list, uint32_t* __restrict__ count
     const size_t stride = (size_t)gridDim.x * blockDim.x;
     for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += stride) list[p] = (uint32_t)p;
     if (blockIdx.x == 0 && threadIdx.x == 0) *count = n;
-}
-
-// perm[dest[p]] = p (only when the caller asks for the permutation)
-__global__ void __launch_bounds__(256)
-k_perm_from_dest(uint32_t n, const uint32_t* __restrict__ dest, uint32_t* __restrict__ perm)
-{
-    const size_t stride = (size_t)gridDim.x * blockDim.x;
-    for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += stride) perm[dest[p]] = (uint32_t)p;
 }
