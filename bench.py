@@ -71,6 +71,8 @@ def parse_args():
     ap.add_argument("--scale", default=None, help="nx,ny,nz override of the grid (tests / quick runs)")
     ap.add_argument("--variant", default="fused", choices=["fused", "atomic"])
     ap.add_argument("--fused-warps", type=int, default=-1, help="8 / 12 / 16 warps per CTA of the fused kernel (library default 12)")
+    ap.add_argument("--m-layout", type=int, default=27, choices=[27, 14],
+                    help="mass-matrix storage: 27 slots per node (north-star, default) or the paper's 14 (L73)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -275,7 +277,8 @@ def run_product(args):
     ctx.enable_timing(True)
     rho = torch.empty(nsp, cfg.nodes, dtype=torch.float64, device=dev)
     J = torch.empty(nsp, 3, cfg.nodes, dtype=torch.float64, device=dev)
-    M = torch.empty(cfg.nodes, 27, 3, 3, dtype=torch.float64, device=dev)
+    ctx.set_m_layout(pk.M_14 if args.m_layout == 14 else pk.M_27)
+    M = torch.empty(cfg.nodes, args.m_layout, 3, 3, dtype=torch.float64, device=dev)
     sorted_input = not cfg.shuffled
 
     def restore_arrays():
@@ -338,7 +341,7 @@ def run_product(args):
         "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {
-            "workload": workload_name(cfg), "particles": n_total, "variant": args.variant,
+            "workload": workload_name(cfg), "particles": n_total, "variant": args.variant, "m_slots": args.m_layout,
             "multi_gpu": "replicas only (north_star: single GPU; each rank runs the whole workload)",
             "l2": "inputs (>= 15 GB at configs[2]) exceed the 126 MB L2; no explicit flush" if n_total * 56 > 2e9
                   else "working set may fit L2 (small config): not a headline number",
@@ -467,9 +470,10 @@ def run_e2e(args, cfg, ctx_unused, pristine, E, B, world):
     Eh, Bh = E.cpu().pin_memory(), B.cpu().pin_memory()
     rho = torch.empty(nsp, cfg.nodes, dtype=torch.float64).pin_memory()
     J = torch.empty(nsp, 3, cfg.nodes, dtype=torch.float64).pin_memory()
-    M = torch.empty(cfg.nodes, 27, 3, 3, dtype=torch.float64).pin_memory()
+    M = torch.empty(cfg.nodes, args.m_layout, 3, 3, dtype=torch.float64).pin_memory()
     ctx = pk.Ecsim(*grid_of(cfg), nsp)
     ctx.set_workspace_host_all(max(n_s), sum(n_s))
+    ctx.set_m_layout(pk.M_14 if args.m_layout == 14 else pk.M_27)
     if args.variant == "atomic":
         ctx.set_variant(pk.VARIANT_ATOMIC)
     qoms = [sp.qom for sp in cfg.species]
@@ -496,7 +500,7 @@ def run_e2e(args, cfg, ctx_unused, pristine, E, B, world):
     n_total = sum(n_s)
     nodes = cfg.nodes
     h2d = sum(7 * 8 * n for n in n_s) + 6 * 8 * nodes
-    d2h = sum(6 * 8 * n for n in n_s) + (243 + 4 * nsp) * 8 * nodes
+    d2h = sum(6 * 8 * n for n in n_s) + (9 * args.m_layout + 4 * nsp) * 8 * nodes
     return {"value": world * n_total * len(times) / t, "unit": UNIT, "h2d_bytes_per_step": h2d,
             "d2h_bytes_per_step": d2h, "steps": len(times),
             "api": "ecsim_push_and_moments_host_all (all species in one call), pinned host memory, copies inside the timed region"}
