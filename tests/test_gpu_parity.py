@@ -440,3 +440,49 @@ def test_pipelined_host_step_rejects_unsorted_input_declared_sorted():
     oracle.step(grid_of(cfg), cfg.species[0].qom, cfg.dt, pn, E.numpy(), B.numpy(), mom)
     assert_moments_close(rho, J, M, mom, "host step, unsorted")
     ctx.close()
+
+
+@pytest.mark.parametrize("warps", [8, 16])
+def test_other_warp_counts_of_the_fused_kernel(warps):
+    """ecsim_set_fused_warps: the 8 x 224- and 16 x 128-register instantiations of the fused kernel (default 12 x 168)."""
+    cfg = wl.config(3, (6, 48, 6))
+    E, B, parts = gen_all(cfg)
+    parts_np = [to_numpy(p) for p in parts]
+    parts_cuda = [to_cuda(p) for p in parts]
+    ctx = make_ctx(cfg, max(p["n"] for p in parts))
+    ctx.set_fused_warps(warps)
+    with pytest.raises(pk.EcsimError, match="invalid"):
+        ctx.set_fused_warps(13)
+    for s, sp in enumerate(cfg.species):
+        ctx.load_particles(s, sp.qom, parts_cuda[s], sorted=True)
+    rho, J, M = alloc_moments(cfg.nodes, 2)
+    ctx.push_and_moments_all(E, B, cfg.dt, cfg.theta, rho, J, M)
+    torch.cuda.synchronize()
+    (total, per_species), = oracle_run(cfg, parts_np, E, B)
+    for s in range(2):
+        assert_particles_close(parts_cuda[s], parts_np[s], cfg, f"species {s}")
+        assert_moments_close(rho[s], J[s], None, per_species[s], f"species {s}")
+    assert_moments_close(None, None, M, total, f"{warps} warps")
+    ctx.close()
+
+
+def test_pipelined_host_step_with_some_outputs_absent():
+    """NULL outputs are skipped in the pipeline too: only rho, then only M."""
+    cfg = wl.config(0)
+    E, B = wl.gen_fields(cfg)
+    part = wl.gen_species(cfg, 0)
+    for want in ("rho", "M"):
+        pn = to_numpy(part)
+        host = {k: part[k].clone().pin_memory() for k in PKEYS}
+        ctx = pk.Ecsim(*grid_of(cfg), 1)
+        ctx.set_workspace(part["n"], host_step=True)
+        ctx.set_host_pipeline(2)
+        rho = torch.full((cfg.nodes,), float("nan"), dtype=torch.float64).pin_memory() if want == "rho" else None
+        M = torch.full((cfg.nodes, 27, 3, 3), float("nan"), dtype=torch.float64).pin_memory() if want == "M" else None
+        ctx.push_and_moments_host(cfg.species[0].qom, True, host, E.contiguous(), B.contiguous(), cfg.dt, cfg.theta, rho, None, M)
+        assert ctx.host_pipelined_count() == 1
+        mom = oracle.Moments(cfg.nodes)
+        oracle.step(grid_of(cfg), cfg.species[0].qom, cfg.dt, pn, E.numpy(), B.numpy(), mom)
+        assert_particles_close(host, pn, cfg, "host step")
+        assert_moments_close(rho, None, M, mom, f"host step, only {want}")
+        ctx.close()
