@@ -47,6 +47,7 @@ struct Resident {
     double slack = 0.25;
     double* buf[2][7] = {};         // two buffers of x,y,z,u,v,w,q
     uint32_t* seg = nullptr;        // [cells+1] first slot of every cell's segment (both buffers)
+    uint32_t* seg_alt = nullptr;    // [cells+1] the table a fresh layout is written to (then the two swap)
     uint32_t* F[2] = {};            // [cells] front runs
     uint32_t* R[2] = {};            // [cells] back runs (arrivals of the last push)
     int cur = 0;                    // buffer that holds the species now
@@ -349,7 +350,7 @@ extern "C" int ecsim_load_particles(ecsim_ctx* c, int s, int64_t n, double q_ove
 }
 
 static int resident_settle(ecsim_ctx* c, int s);
-static int resident_relayout(ecsim_ctx* c, int s);
+static int resident_relayout(ecsim_ctx* c, int s, bool binned);
 
 // Reduced dimensionality (L123 fixPosition): from now on every push pins the coordinates of the axes in axis_mask
 // (bit 0 x, 1 y, 2 z) to the given values; species already loaded are pinned now.
@@ -377,8 +378,8 @@ extern "C" int ecsim_set_fixed_axes(ecsim_ctx* c, int axis_mask, double px, doub
                 CK_LAUNCH();
                 c->launches++;
             }
-            // the pinned particles may now sit in other cells than their segments say: lay the species out afresh
-            rc = resident_relayout(c, s);
+            // the pinned particles may now sit in other cells than their segments say: bin and lay out afresh
+            rc = resident_relayout(c, s, false);
             if (rc) return rc;
         } else {
             k_fix_position<<<grid_for(c, (size_t)sp.n, 256, 16), 256, 0, c->stream>>>(c->g, (size_t)sp.n, sp.x, sp.y, sp.z);
@@ -551,7 +552,7 @@ extern "C" int ecsim_cell_index(ecsim_ctx* c, int s, int32_t* cell_out)
 static size_t resident_tables_bytes(const ecsim_ctx* c, uint32_t ovf_cap)
 {
     const size_t cells = (size_t)c->g.nodes;
-    return align_up(sizeof(uint32_t) * (cells + 1), 256) + 4 * align_up(sizeof(uint32_t) * cells, 256) + 2 * 256 +
+    return 2 * align_up(sizeof(uint32_t) * (cells + 1), 256) + 4 * align_up(sizeof(uint32_t) * cells, 256) + 2 * 256 +
            2 * align_up(sizeof(double) * 7 * (size_t)ovf_cap, 256);
 }
 
@@ -636,20 +637,57 @@ static int resident_export(ecsim_ctx* c, int s, double* const dst[7], bool with_
     return ECSIM_OK;
 }
 
-// a push found segments full: export everything (+ the overflow list) to the idle buffer, lay out afresh
-static int resident_relayout(ecsim_ctx* c, int s)
+// A fresh layout of a resident species (its overflow list has cost more than this does; or fixPosition moved everybody).
+// binned = true: every stored particle is in the cell whose segment holds it (the normal case): only the segments move --
+// new capacities from the cells' totals (+ the homeless particles), a new segment table, one cell-by-cell copy into the
+// idle buffer (15 GB of traffic at configs[2], ~3 ms) and the homeless particles into their cells' back runs.
+// binned = false: export to the idle buffer as dense arrays, bin again, scatter back (three passes).
+static int resident_relayout(ecsim_ctx* c, int s, bool binned = true)
 {
-    Resident& r = c->sp[s].res;
+    SpeciesHost& sp = c->sp[s];
+    Resident& r = sp.res;
+    Workspace& w = c->ws;
     const int other = 1 - r.cur;
-    int rc = resident_export(c, s, r.buf[other], true);
-    if (rc) return rc;
-    const double* src[7];
-    for (int k = 0; k < 7; ++k) src[k] = r.buf[other][k];
-    rc = resident_layout_from_dense(c, s, src, r.cur);
-    if (rc) return rc;
+    const uint32_t cells = (uint32_t)c->g.nodes;
+    const int cgrid = (int)((cells + 255) / 256);
+    int rc;
+    if (!binned) {
+        rc = resident_export(c, s, r.buf[other], true);
+        if (rc) return rc;
+        const double* src[7];
+        for (int k = 0; k < 7; ++k) src[k] = r.buf[other][k];
+        rc = resident_layout_from_dense(c, s, src, r.cur);
+        if (rc) return rc;
+    } else {
+        const double* list = r.ovf[r.ovf_cur];
+        const uint32_t* list_n = r.ovf_count[r.ovf_cur];
+        k_run_totals<<<cgrid, 256, 0, c->stream>>>(cells, r.F[r.cur], r.R[r.cur], w.count);
+        CK_LAUNCH();
+        k_count_list<<<c->sm_count * 2, 256, 0, c->stream>>>(c->g, list_n, r.ovf_cap, list, w.count);
+        CK_LAUNCH();
+        uint32_t* cap = r.R[other];              // scratch until the runs are written
+        k_gapped_caps<<<cgrid, 256, 0, c->stream>>>(cells, w.count, r.slack, RESIDENT_MIN_SLACK, (double)sp.n / (double)cells, cap);
+        CK_LAUNCH();
+        c->launches += 3;
+        rc = scan_u32(c, cap, r.seg_alt, cells);
+        if (rc) return rc;
+        uint32_t total = 0;
+        CK(cudaMemcpyAsync(&total, r.seg_alt + cells, sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream));
+        CK(cudaStreamSynchronize(c->stream));
+        if (total > r.cap_bound) return ECSIM_ERR_WORKSPACE;
+        Soa7c in; Soa7 out;
+        for (int k = 0; k < 7; ++k) { in.a[k] = r.buf[r.cur][k]; out.a[k] = r.buf[other][k]; }
+        k_copy_gapped<<<c->sm_count * 8, 256, 0, c->stream>>>(cells, r.seg, r.F[r.cur], r.R[r.cur], r.seg_alt, r.F[other], r.R[other], in, out);
+        CK_LAUNCH();
+        k_place_list<<<c->sm_count * 2, 256, 0, c->stream>>>(c->g, list_n, r.ovf_cap, list, r.seg_alt, r.R[other], out);
+        CK_LAUNCH();
+        c->launches += 2;
+        uint32_t* t = r.seg; r.seg = r.seg_alt; r.seg_alt = t;
+        r.cur = other;
+    }
     CK(cudaMemsetAsync(r.ovf_count[0], 0, sizeof(uint32_t), c->stream));
     CK(cudaMemsetAsync(r.ovf_count[1], 0, sizeof(uint32_t), c->stream));
-    c->sp[s].stray_debt = 0.0;
+    sp.stray_debt = 0.0;
     c->h_ovf[s] = 0;
     c->relayouts++;
     return ECSIM_OK;
@@ -672,6 +710,7 @@ extern "C" int ecsim_make_resident(ecsim_ctx* c, int s, void* dev_buf, size_t by
     if (bytes < tables + 14 * 256) return ECSIM_ERR_WORKSPACE;
     Carver k{reinterpret_cast<char*>(dev_buf)};
     r.seg = k.take<uint32_t>(cells + 1);
+    r.seg_alt = k.take<uint32_t>(cells + 1);
     r.F[0] = k.take<uint32_t>(cells); r.F[1] = k.take<uint32_t>(cells);
     r.R[0] = k.take<uint32_t>(cells); r.R[1] = k.take<uint32_t>(cells);
     r.ovf_count[0] = k.take<uint32_t>(1);
@@ -714,7 +753,7 @@ static int resident_settle(ecsim_ctx* c, int s)
     sp.leavers_pending = false;
     if (c->h_ovf[s] > sp.res.ovf_cap) return ECSIM_ERR_OVERFLOW;
     sp.stray_debt += (double)c->h_ovf[s];
-    if (c->h_ovf[s] > 0 && sp.stray_debt > 0.25 * c->resort_fraction * (double)sp.n) return resident_relayout(c, s);   // (a homeless particle costs ~4x a stray)
+    if (c->h_ovf[s] > 0 && sp.stray_debt > 0.25 * c->resort_fraction * (double)sp.n) return resident_relayout(c, s, true);   // (a homeless particle costs ~4x a stray)
     return ECSIM_OK;
 }
 

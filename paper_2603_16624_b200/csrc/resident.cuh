@@ -83,3 +83,55 @@ k_append_overflow(const uint32_t* __restrict__ count, uint32_t ovf_cap, const do
         for (int k = 0; k < 7; ++k) dst.a[k][b + i] = ovf[(size_t)k * ovf_cap + i];
     }
 }
+
+// ---- a fresh layout straight from the gapped buffer (the particles are binned already: only the segments move) ----
+// cell of every particle of an overflow list, added to the per-cell totals
+__global__ void __launch_bounds__(256)
+k_count_list(Geom g, const uint32_t* __restrict__ n_ptr, uint32_t cap, const double* __restrict__ list,
+             uint32_t* __restrict__ count)
+{
+    const uint32_t n = min(*n_ptr, cap);
+    const size_t stride = (size_t)gridDim.x * blockDim.x, m = cap;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const int ci = lower_node(list[i] * g.rdx, g.nx), cj = lower_node(list[m + i] * g.rdy, g.ny),
+                  ck = lower_node(list[2 * m + i] * g.rdz, g.nz);
+        atomicAdd(&count[(ci * g.ny + cj) * g.nz + ck], 1u);
+    }
+}
+
+// old segments (front + back runs) -> front runs of the new segments in the other buffer; F_new = F + R, R_new = 0
+__global__ void __launch_bounds__(256)
+k_copy_gapped(uint32_t cells, const uint32_t* __restrict__ seg, const uint32_t* __restrict__ F,
+              const uint32_t* __restrict__ R, const uint32_t* __restrict__ seg_new, uint32_t* __restrict__ F_new,
+              uint32_t* __restrict__ R_new, Soa7c src, Soa7 dst)
+{
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
+    for (uint32_t c = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; c < cells; c += warps) {
+        const uint32_t s0 = seg[c], s1 = seg[c + 1], nf = F[c], nt = nf + R[c], d0 = seg_new[c];
+        for (uint32_t v = lane; v < nt; v += 32u) {
+            const uint32_t p = v < nf ? s0 + v : s1 - 1u - (v - nf);
+#pragma unroll
+            for (int k = 0; k < 7; ++k) dst.a[k][d0 + v] = src.a[k][p];
+        }
+        if (lane == 0) { F_new[c] = nt; R_new[c] = 0u; }
+    }
+}
+
+// the particles of an overflow list into the back runs of the new segments (room is certain: the new capacities
+// counted them)
+__global__ void __launch_bounds__(256)
+k_place_list(Geom g, const uint32_t* __restrict__ n_ptr, uint32_t cap, const double* __restrict__ list,
+             const uint32_t* __restrict__ seg_new, uint32_t* __restrict__ R_new, Soa7 dst)
+{
+    const uint32_t n = min(*n_ptr, cap);
+    const size_t stride = (size_t)gridDim.x * blockDim.x, m = cap;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const int ci = lower_node(list[i] * g.rdx, g.nx), cj = lower_node(list[m + i] * g.rdy, g.ny),
+                  ck = lower_node(list[2 * m + i] * g.rdz, g.nz);
+        const uint32_t c = (uint32_t)((ci * g.ny + cj) * g.nz + ck);
+        const uint32_t pos = seg_new[c + 1] - 1u - atomicAdd(&R_new[c], 1u);
+#pragma unroll
+        for (int k = 0; k < 7; ++k) dst.a[k][pos] = list[(size_t)k * m + i];
+    }
+}

@@ -260,3 +260,80 @@ def test_config2_full_size_second_step_strays_and_resort():
     # the re-sort of a nearly sorted 134 M-particle species (nearly_sorted branch of ecsim_sort_particles)
     _check_sort_bit_exact(cfg, ctx, 0, parts[0], "config 2 electrons after two pushes")
     ctx.close()
+
+
+# ------------------------------------------------------------------ configs[2], resident species: second sort-preserving step
+
+def test_config2_full_size_resident_second_step():
+    """configs[2] at full size with RESIDENT species: after one sort-preserving push (3.1 M particles moved
+    to their new cells' segments) the second step is compared with the oracle on sampled 3x3x3 blocks; zero strays, zero
+    re-sorts, the particle set conserved (ids in the low bits of q), charge conserved on the whole grid."""
+    _need(110)
+    cfg = wl.config(2)
+    E, B, parts = _gen_on_device(cfg)
+    nsp = len(cfg.species)
+    n_s = [int(p["x"].numel()) for p in parts]
+    q0 = [sp.q_sign * cfg.q_abs for sp in cfg.species]
+    for s in range(nsp):
+        parts[s]["q"] = q0[s] * (1.0 + torch.arange(n_s[s], dtype=torch.float64, device="cuda") * 2.0 ** -30)
+    ctx = pk.Ecsim(*grid_of(cfg), nsp)
+    ctx.set_workspace(max(n_s))
+    for s, sp in enumerate(cfg.species):
+        ctx.load_particles(s, sp.qom, parts[s], sorted=True)
+        ctx.make_resident(s, 0.25)
+    rho = torch.empty(nsp, cfg.nodes, dtype=torch.float64, device="cuda")
+    J = torch.empty(nsp, 3, cfg.nodes, dtype=torch.float64, device="cuda")
+    M = torch.empty(cfg.nodes, 27, 3, 3, dtype=torch.float64, device="cuda")
+    ctx.push_and_moments_all(E, B, cfg.dt, cfg.theta, rho, J, M, accumulate=pk.ACC_NONE)
+    torch.cuda.synchronize()
+    assert ctx.stray_count() == 0 and ctx.leaver_count() > 1_000_000
+    # the state after step 1, cell-ordered; the particles that sit in the sampled blocks now
+    blocks = [(40, 77, 3), (126, 126, 126)]
+    befores, ids = {}, {}
+    cur = {k: torch.empty(max(n_s), dtype=torch.float64, device="cuda") for k in PKEYS}
+    for s in range(nsp):
+        ctx.export_particles(s, cur)
+        torch.cuda.synchronize()
+        ci = torch.clamp(torch.floor(cur["x"][:n_s[s]] / cfg.dx), 0, cfg.nx - 1).to(torch.int32)
+        cj = torch.clamp(torch.floor(cur["y"][:n_s[s]] / cfg.dy), 0, cfg.ny - 1).to(torch.int32)
+        ck = torch.clamp(torch.floor(cur["z"][:n_s[s]] / cfg.dz), 0, cfg.nz - 1).to(torch.int32)
+        cell = (ci * cfg.ny + cj) * cfg.nz + ck
+        del ci, cj, ck
+        for o in blocks:
+            want = torch.tensor(_block_cells(cfg, o), dtype=torch.int32, device="cuda")
+            sel = torch.nonzero(torch.isin(cell, want)).flatten()
+            b = {k: cur[k][sel].cpu().numpy().copy() for k in PKEYS}
+            befores.setdefault(o, []).append(b)
+            ids.setdefault(o, []).append(np.rint((b["q"] / q0[s] - 1.0) * 2.0 ** 30).astype(np.int64))
+        del cell
+    rho.fill_(float("nan")); J.fill_(float("nan")); M.fill_(float("nan"))
+    ctx.push_and_moments_all(E, B, cfg.dt, cfg.theta, rho, J, M, accumulate=pk.ACC_NONE)
+    torch.cuda.synchronize()
+    assert ctx.stray_count() == 0 and ctx.resort_count() == 0
+    V = cfg.dx * cfg.dy * cfg.dz
+    after = []
+    for s in range(nsp):
+        ctx.export_particles(s, cur)
+        torch.cuda.synchronize()
+        got_id = torch.round((cur["q"][:n_s[s]] / q0[s] - 1.0) * 2.0 ** 30).to(torch.int64)
+        order = torch.argsort(got_id)
+        assert bool((got_id[order] == torch.arange(n_s[s], device="cuda")).all()), "particle set not conserved"
+        after.append({o: {k: cur[k][:n_s[s]][order[torch.from_numpy(ids[o][s]).cuda()]].cpu().numpy() for k in PKEYS} for o in blocks})
+        del got_id, order
+        qsum = float(cur["q"][:n_s[s]].sum())
+        assert abs(float(rho[s].sum()) * V - qsum) <= 1e-11 * abs(qsum)
+    En, Bn = E.cpu().numpy(), B.cpu().numpy()
+    for o in blocks:
+        nodes = _inner_nodes(cfg, o)
+        total = oracle.Moments(cfg.nodes)
+        for s, sp in enumerate(cfg.species):
+            m = oracle.Moments(cfg.nodes)
+            oracle.step(grid_of(cfg), sp.qom, cfg.dt, befores[o][s], En, Bn, m)
+            assert np.all(np.abs(rho[s, nodes].cpu().numpy() - m.rho[nodes]) <= MOM_TOL * m.rho_abs[nodes])
+            assert np.all(np.abs(J[s][:, nodes].cpu().numpy() - m.J[:, nodes]) <= MOM_TOL * m.J_abs[:, nodes])
+            total.M[nodes] += m.M[nodes]
+            total.M_abs[nodes] += m.M_abs[nodes]
+            assert_particles_close(after[s][o], befores[o][s], cfg, f"resident step 2 block {o} species {s}")
+        got_M = M[nodes].cpu().numpy()
+        assert np.all(np.abs(got_M - total.M[nodes]) <= MOM_TOL * total.M_abs[nodes])
+    ctx.close()
