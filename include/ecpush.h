@@ -70,9 +70,10 @@ enum ecsim_m_layout {
 enum ecsim_variant {
     ECSIM_VARIANT_ATOMIC = 0, /* the paper's design (L143): one thread per particle, one global atomic per
                                  scalar contribution; correct for any particle order                    */
-    ECSIM_VARIANT_FUSED = 1   /* default: cell-sorted particles, one warp per cell, per-cell register accumulators
-                                 (27 weight-product classes x 9 + Jhat + rho) written once per cell with plain
-                                 stores and expanded to the node arrays; strays are added to the per-cell accumulators of their true cell */
+    ECSIM_VARIANT_FUSED = 1   /* default: cell-ordered particles, a warp per contiguous range of cells, per-cell register
+                                 accumulators (27 weight-product classes x 9 + Jhat + rho, pre-reduced on the FP64 matrix
+                                 path) written once per cell with plain stores and expanded to the node arrays; strays
+                                 are added to the per-cell accumulators of their true cell */
 };
 
 /* Create a context for a periodic grid of nx*ny*nz cells (each >= 2) with spacing dx,dy,dz (> 0).
@@ -82,7 +83,7 @@ int ecsim_init_grid(ecsim_ctx **ctx, int nx, int ny, int nz, double dx, double d
 
 /* Scratch bytes needed for species holding at most n_particles_max particles each: per-species cell segment
  * tables, sort keys / ranks / permutation, seven spare arrays for the out-of-place permutation, stray lists,
- * and the per-cell accumulator arrays AM[cells][27][9], AJ[n_species][cells][8][4] of the fused kernel. */
+ * and the per-cell accumulator arrays AM[cells][244], AJ[n_species][cells][8][4] of the fused kernel. */
 size_t ecsim_workspace_bytes(const ecsim_ctx *ctx, int64_t n_particles_max);
 
 /* Lend device scratch (256-byte aligned).  Host-only call. */
@@ -95,6 +96,11 @@ int ecsim_set_workspace(ecsim_ctx *ctx, void *dev_ptr, size_t bytes);
 int ecsim_load_particles(ecsim_ctx *ctx, int species, int64_t n, double q_over_m,
                          double *x, double *y, double *z, double *u, double *v, double *w, double *q,
                          int sorted);
+
+/* Number of particles of a (non-resident) species that the hot path cannot take: a non-finite position, velocity or
+ * charge, or a position outside [0, L) (ecsim_load_particles does not look at the data; positions are expected
+ * wrapped).  Synchronises the stream.  Returns the count (0 = all fine) or a negative ecsim_status. */
+int64_t ecsim_validate_particles(ecsim_ctx *ctx, int species);
 
 /* Counting sort of the species by cell id (L149: the sort the paper could not realise with OpenACC).
  * On return (stream-ordered) the caller's arrays hold the particles grouped by cell, cells ascending;

@@ -50,6 +50,7 @@ _PROTOS = {
     "ecsim_set_workspace": (_c.c_int, [_P, _P, _c.c_size_t]),
     "ecsim_load_particles": (_c.c_int, [_P, _c.c_int, _c.c_int64, _c.c_double] + [_P] * 7 + [_c.c_int]),
     "ecsim_sort_particles": (_c.c_int, [_P, _c.c_int, _P, _P]),
+    "ecsim_validate_particles": (_c.c_int64, [_P, _c.c_int]),
     "ecsim_build_segments": (_c.c_int, [_P, _c.c_int]),
     "ecsim_cell_index": (_c.c_int, [_P, _c.c_int, _P]),
     "ecsim_push_and_moments": (_c.c_int, [_P, _c.c_int, _P, _P, _c.c_double, _c.c_double, _P, _P, _P, _c.c_int]),
@@ -181,6 +182,12 @@ class Ecsim:
         self._resident.pop(species, None)
         _check(self.L.ecsim_load_particles(self.h, species, n, qom, *ptrs, 1 if sorted else 0),
                "ecsim_load_particles")
+
+    def validate_particles(self, species: int) -> int:
+        n = int(self.L.ecsim_validate_particles(self.h, species))
+        if n < 0:
+            _check(n, "ecsim_validate_particles")
+        return n
 
     def sort_particles(self, species: int, cell_count_out=None, perm_out=None):
         _check(self.L.ecsim_sort_particles(self.h, species, _dptr(cell_count_out, self.torch.int32),

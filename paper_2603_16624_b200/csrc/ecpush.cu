@@ -777,6 +777,28 @@ extern "C" int ecsim_export_particles(ecsim_ctx* c, int s, double* x, double* y,
     return resident_export(c, s, dst, true);      // the particles without a slot follow the cell-ordered ones
 }
 
+// Number of particles of a dense species the hot path cannot take: non-finite x, v or q, or a position outside [0, L).
+// Synchronises the stream.  < 0: an ecsim_status.
+extern "C" int64_t ecsim_validate_particles(ecsim_ctx* c, int s)
+{
+    int rc = check_species(c, s);
+    if (rc) return rc;
+    SpeciesHost& sp = c->sp[s];
+    if (sp.res.on) return ECSIM_ERR_INVALID_ARG;
+    rc = need_workspace(c, 0);
+    if (rc) return rc;
+    if (sp.n == 0) return 0;
+    unsigned long long* bad = c->ws.leavers + s;          // (a counter of the workspace that is idle between steps)
+    if (cudaMemsetAsync(bad, 0, sizeof(unsigned long long), c->stream) != cudaSuccess) return ECSIM_ERR_CUDA;
+    k_validate<<<grid_for(c, (size_t)sp.n, 256, 16), 256, 0, c->stream>>>(c->g, (size_t)sp.n, sp.x, sp.y, sp.z, sp.u, sp.v, sp.w, sp.q, bad);
+    if (cudaGetLastError() != cudaSuccess) return ECSIM_ERR_CUDA;
+    c->launches += 2;
+    unsigned long long h = 0;
+    if (cudaMemcpyAsync(&h, bad, sizeof(h), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) return ECSIM_ERR_CUDA;
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return ECSIM_ERR_CUDA;
+    return (int64_t)h;
+}
+
 extern "C" int64_t ecsim_relayout_count(const ecsim_ctx* c) { return c ? c->relayouts : 0; }
 extern "C" int64_t ecsim_host_pipelined_count(const ecsim_ctx* c) { return c ? c->host_pipelined_calls : 0; }
 extern "C" int ecsim_set_host_pipeline(ecsim_ctx* c, int on)

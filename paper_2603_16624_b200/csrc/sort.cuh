@@ -328,3 +328,21 @@ k_iota_u32(uint32_t n, uint32_t* __restrict__ list, uint32_t* __restrict__ count
     for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += stride) list[p] = (uint32_t)p;
     if (blockIdx.x == 0 && threadIdx.x == 0) *count = n;
 }
+
+// ecsim_validate_particles: particles with a non-finite coordinate, velocity or charge, or a position outside [0, L)
+__global__ void __launch_bounds__(256)
+k_validate(Geom g, size_t n, const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
+           const double* __restrict__ u, const double* __restrict__ v, const double* __restrict__ w,
+           const double* __restrict__ q, unsigned long long* __restrict__ bad)
+{
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    unsigned mine = 0;
+    for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += stride) {
+        const double a = x[p], b = y[p], c = z[p];
+        const bool ok = isfinite(u[p]) && isfinite(v[p]) && isfinite(w[p]) && isfinite(q[p]) &&
+                        a >= 0.0 && a < g.Lx && b >= 0.0 && b < g.Ly && c >= 0.0 && c < g.Lz;   // (NaN fails every compare)
+        mine += ok ? 0u : 1u;
+    }
+    mine = __reduce_add_sync(0xffffffffu, mine);
+    if (lane_id() == 0 && mine) atomicAdd(bad, (unsigned long long)mine);
+}

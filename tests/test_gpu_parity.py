@@ -486,3 +486,19 @@ def test_pipelined_host_step_with_some_outputs_absent():
         assert_particles_close(host, pn, cfg, "host step")
         assert_moments_close(rho, None, M, mom, f"host step, only {want}")
         ctx.close()
+
+
+def test_validate_particles_counts_what_the_path_cannot_take():
+    cfg = wl.config(0, (4, 4, 4))
+    part = to_cuda(wl.gen_species(cfg, 0))
+    ctx = make_ctx(cfg, int(part["x"].numel()), n_species=1)
+    ctx.load_particles(0, -64.0, part, sorted=True)
+    assert ctx.validate_particles(0) == 0
+    part["x"][3] = float("nan")
+    part["y"][5] = cfg.lengths[1]            # == L: outside [0, L)
+    part["z"][7] = -1e-300
+    part["w"][9] = float("inf")
+    part["q"][11] = float("nan")
+    part["x"][11] = float("nan")             # two faults, one particle
+    assert ctx.validate_particles(0) == 5
+    ctx.close()
