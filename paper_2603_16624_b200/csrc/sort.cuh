@@ -187,6 +187,8 @@ k_copy_u32_to_i32(uint32_t m, const uint32_t* __restrict__ in, int32_t* __restri
 //          = 3.5 MB each): L2 hits; the writes are coalesced.
 // Round 1 moved one array per launch pair (14 launches, the bookkeeping re-read 7 times, a separate slot-assignment
 // pass with a random 4-byte scatter): 4.35 ms per 33.5 M particles.  tmp = seven spare arrays of the workspace.
+// (measured in round 2, 33.5 M particles: 4096 x 256 buckets 3.75 ms, 8192 x 256 3.80, 8192 x 512 3.81, 16384 x 512 3.80,
+// 16384 x 256 3.83: the move is not sensitive to the tile / bucket geometry)
 constexpr int SORT_TILE = 8192;
 constexpr int SORT_MAX_BUCKETS = 512;
 constexpr int SORT_STAGE_THREADS = 512;
@@ -234,9 +236,12 @@ k_stage7_to_slots(uint32_t n, const uint32_t* __restrict__ dest, const uint32_t*
     const uint32_t b = threadIdx.x;
     const uint32_t c = b < nb ? H[(size_t)b * tiles + blockIdx.x] : 0u;
     const uint32_t ex = block_exclusive_scan(c, &total);
-    toff[b] = ex;
-    base[b] = b < nb ? Hs[(size_t)b * tiles + blockIdx.x] : 0u;
-    cnt[b] = 0u;
+    static_assert(SORT_MAX_BUCKETS <= SORT_STAGE_THREADS, "one thread per bucket in the tile-local scan");
+    if (b < (uint32_t)SORT_MAX_BUCKETS) {
+        toff[b] = ex;
+        base[b] = b < nb ? Hs[(size_t)b * tiles + blockIdx.x] : 0u;
+        cnt[b] = 0u;
+    }
     __syncthreads();
     const size_t p0 = (size_t)blockIdx.x * SORT_TILE;
     const uint32_t tile_n = (uint32_t)min((size_t)SORT_TILE, (size_t)n - p0);
