@@ -167,6 +167,7 @@ int ecsim_push_all(ecsim_ctx *ctx, const double *E_theta, const double *B, doubl
  * species) the species is laid out afresh (counted by ecsim_relayout_count).  The arrays given to ecsim_load_particles are not referenced after ecsim_make_resident returns
  * and are NOT updated by pushes: read the species back with ecsim_export_particles (device arrays of n doubles each;
  * cell-major order; also works, as a plain copy, for a species that is not resident).
+ * (A species loaded with sorted = 0 is sorted in place first -- its arrays are permuted -- so that the copy is sequential.)
  * ecsim_make_resident synchronises the stream once (it checks the data-dependent slot count against the buffer);
  * slack in [0, 4], typically 0.25.  All species of one *_all call must be of one kind (all resident or none). */
 size_t ecsim_resident_bytes(const ecsim_ctx *ctx, int64_t n_particles, double slack);
