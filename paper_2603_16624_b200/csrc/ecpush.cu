@@ -81,7 +81,8 @@ struct Workspace {
     int32_t* cell = nullptr;         // [n_max]
     uint32_t* rank = nullptr;        // [n_max]
     uint32_t* perm = nullptr;        // [n_max]
-    double* spare = nullptr;         // [7][n_max]: the seven arrays of a species on their way through a sort
+    double* spare = nullptr;         // [8][n_max]: the seven arrays of a species on their way through a re-sort, or its
+                                     // n_max 64-byte records on their way through a sort of arbitrary order
     uint32_t* tile_hist = nullptr;   // [buckets][tiles] of the two-step move of a random-order sort
     uint32_t* tile_scan = nullptr;   // its exclusive scan (+1)
     uint32_t* tile_sums = nullptr;   // block sums of that scan
@@ -150,7 +151,7 @@ static size_t carve(const ecsim_ctx* c, int64_t n_max, void* base, Workspace* ou
     w.cell = k.take<int32_t>(n);
     w.rank = k.take<uint32_t>(n);
     w.perm = k.take<uint32_t>(n);
-    w.spare = k.take<double>(7 * n);
+    w.spare = k.take<double>(8 * n);
     {
         const size_t m = (size_t)SORT_MAX_BUCKETS * (n / SORT_TILE + 1);
         w.tile_hist = k.take<uint32_t>(m);
@@ -486,8 +487,8 @@ extern "C" int ecsim_sort_particles(ecsim_ctx* c, int s, int32_t* cell_count_out
             if (perm_out)
                 CK(cudaMemcpyAsync(perm_out, w.perm, sizeof(uint32_t) * (size_t)n, cudaMemcpyDeviceToDevice, c->stream));
         } else {
-            // arbitrary order: the bucketed two-step move of sort.cuh, seven arrays per launch
-            CK(cudaFuncSetAttribute(k_stage7_to_slots, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SORT_STAGE_SMEM));
+            // arbitrary order: the bucketed two-step move of sort.cuh through 64-byte records
+            CK(cudaFuncSetAttribute(k_stage_records, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SORT_STAGE_SMEM));
             int shift = 13;
             while ((((n - 1) >> shift) + 1) > (uint32_t)SORT_MAX_BUCKETS) ++shift;
             const uint32_t nbk = ((n - 1) >> shift) + 1;
@@ -495,7 +496,6 @@ extern "C" int ecsim_sort_particles(ecsim_ctx* c, int s, int32_t* cell_count_out
             const uint32_t m = nbk * tiles;
             uint32_t* dest = w.rank;                                   // rank -> dest in place
             uint32_t* tmpdest = w.perm;
-            uint32_t* tmpidx = perm_out ? reinterpret_cast<uint32_t*>(w.cell) : nullptr;   // the cell ids are not needed after dest
             k_dest_and_tile_hist<<<tiles, 256, 0, c->stream>>>(n, w.cell, dest, start, shift, tiles, w.tile_hist);
             CK_LAUNCH();
             const uint32_t sb = (m + SCAN_BLOCK - 1) / SCAN_BLOCK;
@@ -506,18 +506,16 @@ extern "C" int ecsim_sort_particles(ecsim_ctx* c, int s, int32_t* cell_count_out
             k_scan_add<<<sb, SCAN_BLOCK, 0, c->stream>>>(w.tile_scan, w.tile_sums, m);
             CK_LAUNCH();
             Sort7 s7;
-            Move7 mv;
-            for (int a = 0; a < 7; ++a) {
-                s7.in[a] = arrays[a]; s7.tmp[a] = w.spare + a * nmax;
-                mv.src[a] = w.spare + a * nmax; mv.dst[a] = arrays[a];
-            }
-            k_stage7_to_slots<<<tiles, SORT_STAGE_THREADS, SORT_STAGE_SMEM, c->stream>>>(n, dest, w.tile_hist, w.tile_scan, shift,
-                                                                                      tiles, s7, tmpdest, tmpidx);
+            Out7 o7;
+            for (int a = 0; a < 7; ++a) { s7.in[a] = arrays[a]; o7.dst[a] = arrays[a]; }
+            k_stage_records<<<tiles, SORT_STAGE_THREADS, SORT_STAGE_SMEM, c->stream>>>(n, dest, w.tile_hist, w.tile_scan, shift,
+                                                                                    tiles, s7, w.spare, tmpdest);
             CK_LAUNCH();
             uint32_t* perm2 = w.stray_list + (size_t)s * (size_t)w.n_max;      // (the stray lists are idle during a sort)
-            k_invert_slots<<<grid, 256, 0, c->stream>>>(n, tmpdest, perm2, tmpidx, perm_out);
+            k_invert_slots<<<grid, 256, 0, c->stream>>>(n, tmpdest, perm2);
             CK_LAUNCH();
-            k_gather7<<<grid, 256, 0, c->stream>>>(n, perm2, mv);
+            k_gather_records<<<grid_for(c, ((size_t)n + 31) / 32, GATHER_WARPS, 8), GATHER_WARPS * 32, 0, c->stream>>>(
+                n, perm2, w.spare, o7, perm_out);
             CK_LAUNCH();
             c->launches += 7;
         }

@@ -5,7 +5,7 @@
 //   k_scan_*      exclusive scan of the histogram -> start[cells+1]
 //   k_build_perm  perm[start[cell] + rank] = old index
 //   k_gather7     out[new] = in[perm[new]] for the seven SoA arrays (re-sort of a nearly sorted species)
-//   k_stage7_to_slots / k_scatter7  the two-step move of a species in arbitrary order
+//   k_stage_records / k_gather_records  the two-step move of a species in arbitrary order
 //
 // Integer work only; results (cell ids, counts) are bit-exact functions of the stored positions.
 #pragma once
@@ -20,8 +20,11 @@ __device__ __forceinline__ int cell_of(const Geom& g, double x, double y, double
     return (i * g.ny + j) * g.nz + k;
 }
 
-// One thread per particle.  Lanes of a warp that fall in the same cell are aggregated with
-// match_any so that a cell-sorted input costs one atomic per (warp, cell) instead of 32.
+// One thread per particle, HIST_ILP particles per thread and loop pass.  Lanes of a warp that fall in the same cell are
+// aggregated with match_any so that a cell-sorted input costs one atomic per (warp, cell) instead of 32; for an input
+// in arbitrary order every particle pays its own L2 atomic, whose round trip bounds the kernel: the HIST_ILP atomics of
+// a pass are issued before the first result is used.
+constexpr int HIST_ILP = 4;
 template <bool WITH_RANK>
 __global__ void __launch_bounds__(256)
 k_cell_hist(Geom g, uint32_t n, const double* __restrict__ x, const double* __restrict__ y,
@@ -30,18 +33,36 @@ k_cell_hist(Geom g, uint32_t n, const double* __restrict__ x, const double* __re
 {
     const size_t stride = (size_t)gridDim.x * blockDim.x;
     const size_t n_round = ((size_t)n + 31) & ~(size_t)31;   // keep whole warps in the loop
-    for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < n_round; p += stride) {
-        const bool active = p < n;
-        int c = -1;
-        if (active) c = cell_of(g, x[p], y[p], z[p]);
-        const unsigned peers = __match_any_sync(0xffffffffu, c);
-        if (active) {
-            const int leader = __ffs(peers) - 1;
-            uint32_t base = 0;
-            if ((int)lane_id() == leader) base = atomicAdd(&count[c], (uint32_t)__popc(peers));
-            base = __shfl_sync(peers, base, leader);
-            if (cell_out) cell_out[p] = c;
-            if (WITH_RANK) rank_out[p] = base + __popc(peers & ((1u << lane_id()) - 1u));
+    const unsigned lane = lane_id(), lt = (1u << lane) - 1u;
+    for (size_t p0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p0 < n_round; p0 += stride * HIST_ILP) {
+        int c[HIST_ILP];
+        unsigned peers[HIST_ILP];
+        uint32_t base[HIST_ILP];
+#pragma unroll
+        for (int j = 0; j < HIST_ILP; ++j) {
+            const size_t p = p0 + (size_t)j * stride;
+            c[j] = p < n ? cell_of(g, x[p], y[p], z[p]) : -1;
+        }
+#pragma unroll
+        for (int j = 0; j < HIST_ILP; ++j) {
+            const size_t p = p0 + (size_t)j * stride;
+            base[j] = 0;
+            peers[j] = 0;
+            if (p < n_round) {                                // warp-uniform: p - lane is the same multiple of 32 for the warp
+                peers[j] = __match_any_sync(0xffffffffu, c[j]);
+                if (c[j] >= 0 && (int)lane == __ffs(peers[j]) - 1) base[j] = atomicAdd(&count[c[j]], (uint32_t)__popc(peers[j]));
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < HIST_ILP; ++j) {
+            const size_t p = p0 + (size_t)j * stride;
+            if (p < n_round) {
+                const uint32_t b = __shfl_sync(0xffffffffu, base[j], __ffs(peers[j]) - 1);
+                if (c[j] >= 0) {
+                    if (cell_out) cell_out[p] = c[j];
+                    if (WITH_RANK) rank_out[p] = b + __popc(peers[j] & lt);
+                }
+            }
         }
     }
 }
@@ -173,27 +194,27 @@ k_copy_u32_to_i32(uint32_t m, const uint32_t* __restrict__ in, int32_t* __restri
 // ---------------------------------------------------------------------------------------------
 // Moving the seven SoA arrays of a species given in RANDOM order (config 4) to their sorted places.
 // A random 8-byte gather from HBM costs ~97 bytes of traffic on B200 (3.26 GB per 33.5 M elements,
-// profiles/r01d), and scattered 8-byte stores are bound by L2 transactions, so the permutation is applied in
-// two steps that are both local.  dest[p] = start[cell[p]] + rank[p] is the final place of particle p;
+// profiles/r01d), and scattered 8-byte stores are read-modify-writes of their sectors, so the permutation is
+// applied in two steps that are both local.  dest[p] = start[cell[p]] + rank[p] is the final place of particle p;
 // places are cut into <= SORT_MAX_BUCKETS buckets of 2^shift consecutive places (every bucket is full,
 // dest being a permutation).
-//   step A, k_stage7_to_slots: a tile of SORT_TILE particles per CTA.  A particle's slot = (places of its bucket taken
+//   step A, k_stage_records: a tile of SORT_TILE particles per CTA.  A particle's slot = (places of its bucket taken
 //          by earlier tiles, from the scanned per-(bucket, tile) histogram) + (its arrival rank in the tile, a shared-
-//          memory atomic).  The tile is ordered by bucket in shared memory and written to tmp[] in runs of
-//          ~SORT_TILE/buckets consecutive elements: coalesced.  ALL SEVEN arrays go through one launch -- the slot
-//          bookkeeping is computed once, kept in registers, and the final place travels with the particle (tmpdest).
-//   step B, k_invert_slots + k_gather7: perm2 = tmpdest^-1, then out[d] = tmp[perm2[d]] for the seven arrays: a gather
-//          whose sources lie inside the windows of the ~9 buckets in flight (grid-stride; 2^shift places x 7 arrays x 8 B
-//          = 3.5 MB each): L2 hits; the writes are coalesced.
-// Round 1 moved one array per launch pair (14 launches, the bookkeeping re-read 7 times, a separate slot-assignment
-// pass with a random 4-byte scatter): 4.35 ms per 33.5 M particles.  tmp = seven spare arrays of the workspace.
-// (measured in round 2, 33.5 M particles: 4096 x 256 buckets 3.75 ms, 8192 x 256 3.80, 8192 x 512 3.81, 16384 x 512 3.80,
-// 16384 x 256 3.83: the move is not sensitive to the tile / bucket geometry)
-constexpr int SORT_TILE = 8192;
-constexpr int SORT_MAX_BUCKETS = 512;
-constexpr int SORT_STAGE_THREADS = 512;
+//          memory atomic).  The seven values of a particle are read once (coalesced SoA loads, 28 in flight per
+//          thread), put together as ONE 64-byte record {x,y,z,u,v,w,q, (dest, original index)} at the particle's position in
+//          the tile's bucket order in shared memory, and the tile is written to tmp[] in runs of ~SORT_TILE/buckets
+//          whole records: one load phase, one barrier, one store phase per tile (round 2 first moved array by array:
+//          seven load / store phase pairs per tile, 128-byte runs, 1.52 ms per 33.5 M particles at 2.9 TB/s).
+//   step B, k_invert_slots + k_gather_records: perm2 = tmpdest^-1, then place d takes record perm2[d]: four lanes read
+//          one record (two whole sectors; the 8-byte gather of the SoA version fetched seven sectors per particle and
+//          ran at 83 % of the L1 tag rate, ncu), a per-warp transposition in shared memory, seven coalesced stores.
+//          The sources of the places in flight lie inside the windows of a few buckets (2^shift records of 64 B).
+// tmp = eight spare arrays of the workspace.
+constexpr int SORT_TILE = 1024;
+constexpr int SORT_MAX_BUCKETS = 256;
+constexpr int SORT_STAGE_THREADS = 256;
 constexpr int SORT_PER_THREAD = SORT_TILE / SORT_STAGE_THREADS;
-constexpr size_t SORT_STAGE_SMEM = (size_t)SORT_TILE * (sizeof(double) + sizeof(uint32_t)) + 3 * SORT_MAX_BUCKETS * sizeof(uint32_t);
+constexpr size_t SORT_STAGE_SMEM = (size_t)SORT_TILE * (8 * sizeof(double) + sizeof(uint32_t)) + 3 * SORT_MAX_BUCKETS * sizeof(uint32_t);   // 72.7 KB: 3 CTAs per SM
 
 // dest (in place of rank) and the per-(bucket, tile) histogram H[b * tiles + tile]
 __global__ void __launch_bounds__(256)
@@ -217,26 +238,28 @@ k_dest_and_tile_hist(uint32_t n, const int32_t* __restrict__ cell, uint32_t* __r
     for (uint32_t b = threadIdx.x; b < nb; b += blockDim.x) H[(size_t)b * tiles + blockIdx.x] = cnt[b];
 }
 
-struct Sort7 { const double* in[7]; double* tmp[7]; };
+struct Sort7 { const double* in[7]; };
 
-// step A for the seven arrays of one tile.  H: per-(bucket, tile) histogram, Hs: its exclusive scan.
-__global__ void __launch_bounds__(SORT_STAGE_THREADS)
-k_stage7_to_slots(uint32_t n, const uint32_t* __restrict__ dest, const uint32_t* __restrict__ H,
-                  const uint32_t* __restrict__ Hs, int shift, uint32_t tiles, Sort7 a, uint32_t* __restrict__ tmpdest,
-                  uint32_t* __restrict__ tmpidx /* or null */)
+// step A: the records of one tile.  H: per-(bucket, tile) histogram, Hs: its exclusive scan.  In shared memory word k of
+// the record at tile position lp sits at lp*8 + (k ^ (lp & 7)): the writes of a warp (one k, scattered lp) spread over
+// the banks, the 16-byte reads of the store phase stay aligned pairs (swapped where lp is odd).
+__global__ void __launch_bounds__(SORT_STAGE_THREADS, 3)
+k_stage_records(uint32_t n, const uint32_t* __restrict__ dest, const uint32_t* __restrict__ H,
+                const uint32_t* __restrict__ Hs, int shift, uint32_t tiles, Sort7 a, double* __restrict__ tmp,
+                uint32_t* __restrict__ tmpdest)
 {
     extern __shared__ __align__(16) unsigned char stage_smem[];
-    double* vals = reinterpret_cast<double*>(stage_smem);
-    uint32_t* dsts = reinterpret_cast<uint32_t*>(vals + SORT_TILE);   // slot of the element at tile position lp
-    uint32_t* base = dsts + SORT_TILE;          // first slot of this tile's share of bucket b
+    double* rec = reinterpret_cast<double*>(stage_smem);
+    uint32_t* slot = reinterpret_cast<uint32_t*>(rec + (size_t)SORT_TILE * 8);   // slot of the record at tile position lp
+    uint32_t* base = slot + SORT_TILE;          // first slot of this tile's share of bucket b
     uint32_t* toff = base + SORT_MAX_BUCKETS;   // where bucket b starts in the tile's bucket order
     uint32_t* cnt = toff + SORT_MAX_BUCKETS;    // arrivals so far
     __shared__ uint32_t total;
+    static_assert(SORT_MAX_BUCKETS <= SORT_STAGE_THREADS, "one thread per bucket in the tile-local scan");
     const uint32_t nb = ((n - 1) >> shift) + 1;
     const uint32_t b = threadIdx.x;
     const uint32_t c = b < nb ? H[(size_t)b * tiles + blockIdx.x] : 0u;
     const uint32_t ex = block_exclusive_scan(c, &total);
-    static_assert(SORT_MAX_BUCKETS <= SORT_STAGE_THREADS, "one thread per bucket in the tile-local scan");
     if (b < (uint32_t)SORT_MAX_BUCKETS) {
         toff[b] = ex;
         base[b] = b < nb ? Hs[(size_t)b * tiles + blockIdx.x] : 0u;
@@ -245,59 +268,111 @@ k_stage7_to_slots(uint32_t n, const uint32_t* __restrict__ dest, const uint32_t*
     __syncthreads();
     const size_t p0 = (size_t)blockIdx.x * SORT_TILE;
     const uint32_t tile_n = (uint32_t)min((size_t)SORT_TILE, (size_t)n - p0);
-    uint32_t lp[SORT_PER_THREAD];               // this thread's elements: their positions in the tile's bucket order
-    uint32_t* dvals = reinterpret_cast<uint32_t*>(vals);
+    // load phase: all 7 x SORT_PER_THREAD values of this thread are requested before the first is used
+    double v[SORT_PER_THREAD][7];
+    uint32_t d[SORT_PER_THREAD];
 #pragma unroll
     for (int j = 0; j < SORT_PER_THREAD; ++j) {
         const uint32_t e = threadIdx.x + j * SORT_STAGE_THREADS;
-        lp[j] = 0xffffffffu;
         if (e < tile_n) {
-            const uint32_t d = dest[p0 + e], bk = d >> shift;
+            d[j] = dest[p0 + e];
+#pragma unroll
+            for (int k = 0; k < 7; ++k) v[j][k] = a.in[k][p0 + e];
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < SORT_PER_THREAD; ++j) {
+        const uint32_t e = threadIdx.x + j * SORT_STAGE_THREADS;
+        if (e < tile_n) {
+            const uint32_t bk = d[j] >> shift;
             const uint32_t r = atomicAdd(&cnt[bk], 1u);
-            lp[j] = toff[bk] + r;
-            dsts[lp[j]] = base[bk] + r;
-            dvals[lp[j]] = d;
+            const uint32_t lp = toff[bk] + r;
+            slot[lp] = base[bk] + r;
+            double* w = rec + (size_t)lp * 8;
+            const uint32_t sw = lp & 7u;
+#pragma unroll
+            for (int k = 0; k < 7; ++k) w[k ^ sw] = v[j][k];
+            // the original index (low word) and the final place (high word) travel with the record
+            w[7 ^ sw] = __longlong_as_double((long long)(((unsigned long long)d[j] << 32) | (unsigned long long)(p0 + e)));
         }
     }
     __syncthreads();
-    for (uint32_t t = threadIdx.x; t < tile_n; t += SORT_STAGE_THREADS) tmpdest[dsts[t]] = dvals[t];
-    __syncthreads();
-    if (tmpidx) {
-#pragma unroll
-        for (int j = 0; j < SORT_PER_THREAD; ++j)
-            if (lp[j] != 0xffffffffu) dvals[lp[j]] = (uint32_t)(p0 + threadIdx.x + j * SORT_STAGE_THREADS);
-        __syncthreads();
-        for (uint32_t t = threadIdx.x; t < tile_n; t += SORT_STAGE_THREADS) tmpidx[dsts[t]] = dvals[t];
-        __syncthreads();
+    // store phase: 16-byte pieces, consecutive threads = consecutive pieces of consecutive records of a run
+    for (uint32_t t = threadIdx.x; t < tile_n * 4u; t += SORT_STAGE_THREADS) {
+        const uint32_t r = t >> 2, part = t & 3u, sw = r & 7u;
+        double2 pr = *reinterpret_cast<const double2*>(rec + (size_t)r * 8 + ((2u * part) ^ (sw & 6u)));
+        if (sw & 1u) { const double h = pr.x; pr.x = pr.y; pr.y = h; }
+        *reinterpret_cast<double2*>(tmp + (size_t)slot[r] * 8 + 2u * part) = pr;
     }
-#pragma unroll 1
-    for (int k = 0; k < 7; ++k) {
-        const double* __restrict__ in = a.in[k];
-        double* __restrict__ tmp = a.tmp[k];
-#pragma unroll
-        for (int j = 0; j < SORT_PER_THREAD; ++j)
-            if (lp[j] != 0xffffffffu) vals[lp[j]] = in[p0 + threadIdx.x + j * SORT_STAGE_THREADS];
-        __syncthreads();
-        for (uint32_t t = threadIdx.x; t < tile_n; t += SORT_STAGE_THREADS) tmp[dsts[t]] = vals[t];
-        __syncthreads();
-    }
+    for (uint32_t t = threadIdx.x; t < tile_n; t += SORT_STAGE_THREADS)
+        tmpdest[slot[t]] = (uint32_t)((unsigned long long)__double_as_longlong(rec[(size_t)t * 8 + (7u ^ (t & 7u))]) >> 32);
 }
 
 struct Move7 { const double* src[7]; double* dst[7]; };
 
 // step B, first half: the inverse of tmpdest, perm2[tmpdest[t]] = t (a 4-byte scatter that stays inside the bucket's
-// window: L2), and the permutation for the caller if asked.  (Scattering the seven payload arrays the same way was
-// measured: 5.5 ms per 33.5 M particles, every 8-byte store a read-modify-write of its DRAM sector; the gather below
-// reads at random from the L2-resident window instead and writes whole sectors.)
+// window: L2).  (Scattering the payload the same way was measured: 5.5 ms per 33.5 M particles, every 8-byte store a
+// read-modify-write of its DRAM sector; the gather below reads whole records and writes whole sectors.)
 __global__ void __launch_bounds__(256)
-k_invert_slots(uint32_t n, const uint32_t* __restrict__ tmpdest, uint32_t* __restrict__ perm2,
-               const uint32_t* __restrict__ tmpidx, uint32_t* __restrict__ perm_out)
+k_invert_slots(uint32_t n, const uint32_t* __restrict__ tmpdest, uint32_t* __restrict__ perm2)
 {
     const size_t stride = (size_t)gridDim.x * blockDim.x;
-    for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += stride) {
-        const uint32_t d = tmpdest[t];
-        perm2[d] = (uint32_t)t;
-        if (perm_out) perm_out[d] = tmpidx[t];
+    for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += stride) perm2[tmpdest[t]] = (uint32_t)t;
+}
+
+struct Out7 { double* dst[7]; };
+
+// L2 residency hints of the gather: the two records of a 128-byte line are wanted at unrelated moments while their
+// bucket is in flight, so the record loads ask to be evicted last and everything streamed (places, outputs) first
+// (without the hints the records were fetched from DRAM 1.7 times each, ncu dram__bytes_read)
+__device__ __forceinline__ unsigned long long l2_policy_evict_last()
+{
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ double2 ld_evict_last_f64x2(const double* p, unsigned long long pol)
+{
+    double2 v;
+    asm volatile("ld.global.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol));
+    return v;
+}
+
+// step B, second half: place d takes record perm2[d].  A warp owns 32 consecutive places; lanes 4j..4j+3 read the four
+// 16-byte pieces of one record (8 records per load instruction), the warp transposes through shared memory (pitch 9:
+// conflict-free) and writes the seven arrays (and the permutation, if asked) coalesced.
+constexpr int GATHER_WARPS = 8;
+__global__ void __launch_bounds__(GATHER_WARPS * 32)
+k_gather_records(uint32_t n, const uint32_t* __restrict__ perm2, const double* __restrict__ tmp, Out7 a,
+                 uint32_t* __restrict__ perm_out /* or null */)
+{
+    __shared__ double stage[GATHER_WARPS][32 * 9];
+    const unsigned lane = lane_id(), warp = threadIdx.x >> 5;
+    double* st = stage[warp];
+    const uint32_t j = lane >> 2, part = lane & 3u;
+    const size_t chunks = ((size_t)n + 31) / 32;
+    const unsigned long long keep = l2_policy_evict_last();
+    for (size_t ch = (size_t)blockIdx.x * GATHER_WARPS + warp; ch < chunks; ch += (size_t)gridDim.x * GATHER_WARPS) {
+        const size_t dp = ch * 32 + lane;
+        const uint32_t q = dp < n ? __ldcs(perm2 + dp) : 0u;
+        double2 pr[4];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const uint32_t src = __shfl_sync(0xffffffffu, q, 8 * r + (int)j);
+            pr[r] = ld_evict_last_f64x2(tmp + (size_t)src * 8 + 2u * part, keep);
+        }
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            double* w = st + (8 * r + j) * 9 + 2 * part;
+            w[0] = pr[r].x; w[1] = pr[r].y;
+        }
+        __syncwarp();
+        if (dp < n) {
+#pragma unroll
+            for (int k = 0; k < 7; ++k) __stcs(a.dst[k] + dp, st[lane * 9 + k]);
+            if (perm_out) __stcs(perm_out + dp, (uint32_t)__double_as_longlong(st[lane * 9 + 7]));
+        }
+        __syncwarp();
     }
 }
 
