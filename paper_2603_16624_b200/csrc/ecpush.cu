@@ -6,6 +6,7 @@
 #include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
+#include <algorithm>
 #include <new>
 
 #include "../../include/ecpush.h"
@@ -83,9 +84,10 @@ struct Workspace {
     uint32_t* perm = nullptr;        // [n_max]
     double* spare = nullptr;         // [8][n_max]: the seven arrays of a species on their way through a re-sort, or its
                                      // n_max 64-byte records on their way through a sort of arbitrary order
-    uint32_t* tile_hist = nullptr;   // [buckets][tiles] of the two-step move of a random-order sort
-    uint32_t* tile_scan = nullptr;   // its exclusive scan (+1)
-    uint32_t* tile_sums = nullptr;   // block sums of that scan
+    uint32_t* tile_hist = nullptr;   // [tiles][SORT_MAX_BUCKETS] of the two-step move of a random-order sort
+    uint32_t* tile_off = nullptr;    // its tile-local exclusive scans over the buckets
+    uint32_t* tile_scan = nullptr;   // first slot of every (tile, bucket) share
+    uint32_t* tile_sums = nullptr;   // [chunks of tiles][SORT_MAX_BUCKETS] column sums
     uint32_t* stray_list = nullptr;  // [n_species][n_max]
     double* AM = nullptr;            // [cells][AM_PER_CELL = 244]
     double* AJ = nullptr;            // [n_species][cells][32]
@@ -155,8 +157,9 @@ static size_t carve(const ecsim_ctx* c, int64_t n_max, void* base, Workspace* ou
     {
         const size_t m = (size_t)SORT_MAX_BUCKETS * (n / SORT_TILE + 1);
         w.tile_hist = k.take<uint32_t>(m);
+        w.tile_off = k.take<uint32_t>(m);
         w.tile_scan = k.take<uint32_t>(m + 1);
-        w.tile_sums = k.take<uint32_t>(m / SCAN_BLOCK + 2);
+        w.tile_sums = k.take<uint32_t>(((n / SORT_TILE + 1) / SORT_CHUNK + 1) * (size_t)SORT_MAX_BUCKETS);
     }
     w.stray_list = k.take<uint32_t>(nsp * n);
     w.AM = k.take<double>(cells * AM_PER_CELL);
@@ -491,30 +494,35 @@ extern "C" int ecsim_sort_particles(ecsim_ctx* c, int s, int32_t* cell_count_out
             CK(cudaFuncSetAttribute(k_stage_records, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SORT_STAGE_SMEM));
             int shift = 13;
             while ((((n - 1) >> shift) + 1) > (uint32_t)SORT_MAX_BUCKETS) ++shift;
-            const uint32_t nbk = ((n - 1) >> shift) + 1;
             const uint32_t tiles = (n + SORT_TILE - 1) / SORT_TILE;
-            const uint32_t m = nbk * tiles;
             uint32_t* dest = w.rank;                                   // rank -> dest in place
             uint32_t* tmpdest = w.perm;
-            k_dest_and_tile_hist<<<tiles, 256, 0, c->stream>>>(n, w.cell, dest, start, shift, tiles, w.tile_hist);
+            uint32_t* perm2 = w.stray_list + (size_t)s * (size_t)w.n_max;      // (the stray lists are idle during a sort)
+            uint32_t* T = w.tile_off;
+            const uint32_t chunks = (tiles + SORT_CHUNK - 1) / SORT_CHUNK;
+            k_dest_and_tile_hist<<<tiles, SORT_MAX_BUCKETS, 0, c->stream>>>(n, w.cell, dest, start, shift, w.tile_hist, T);
             CK_LAUNCH();
-            const uint32_t sb = (m + SCAN_BLOCK - 1) / SCAN_BLOCK;
-            k_scan_blocks<<<sb, SCAN_BLOCK, 0, c->stream>>>(w.tile_hist, w.tile_scan, w.tile_sums, m);
+            k_tile_colsum<<<chunks, SORT_MAX_BUCKETS, 0, c->stream>>>(tiles, w.tile_hist, w.tile_sums);
             CK_LAUNCH();
-            k_scan_sums<<<1, SCAN_BLOCK, 0, c->stream>>>(w.tile_sums, sb, w.tile_scan, m);
+            k_tile_chunkscan<<<1, SORT_MAX_BUCKETS, 0, c->stream>>>(chunks, w.tile_sums);
             CK_LAUNCH();
-            k_scan_add<<<sb, SCAN_BLOCK, 0, c->stream>>>(w.tile_scan, w.tile_sums, m);
+            k_tile_colscan<<<chunks, SORT_MAX_BUCKETS, 0, c->stream>>>(tiles, shift, w.tile_hist, w.tile_sums, w.tile_scan);
             CK_LAUNCH();
             Sort7 s7;
             Out7 o7;
             for (int a = 0; a < 7; ++a) { s7.in[a] = arrays[a]; o7.dst[a] = arrays[a]; }
-            k_stage_records<<<tiles, SORT_STAGE_THREADS, SORT_STAGE_SMEM, c->stream>>>(n, dest, w.tile_hist, w.tile_scan, shift,
-                                                                                    tiles, s7, w.spare, tmpdest);
+            k_stage_records<<<tiles, SORT_STAGE_THREADS, SORT_STAGE_SMEM, c->stream>>>(n, dest, T, w.tile_scan, shift, s7, w.spare,
+                                                                                    tmpdest);
             CK_LAUNCH();
-            uint32_t* perm2 = w.stray_list + (size_t)s * (size_t)w.n_max;      // (the stray lists are idle during a sort)
             k_invert_slots<<<grid, 256, 0, c->stream>>>(n, tmpdest, perm2);
             CK_LAUNCH();
-            k_gather_records<<<grid_for(c, ((size_t)n + 31) / 32, GATHER_WARPS, 8), GATHER_WARPS * 32, 0, c->stream>>>(
+            // the places in flight (one per thread) must span less than one bucket, or the second record of a 128-byte
+            // line arrives after the line has left L2 (measured at 33.5 M particles, buckets of 131,072 places: 3 CTAs per
+            // SM 0.70 ms and 2.28 GB read, 4 per SM 0.94 ms and 3.08 GB); whole multiples of the SM count keep the CTAs abreast
+            int per_sm = 8;
+            if ((size_t)n * 64 > ((size_t)48 << 20))
+                per_sm = (int)std::min<size_t>(8, std::max<size_t>(1, ((size_t)9 << shift) / 10 / (GATHER_WARPS * 32) / (size_t)c->sm_count));
+            k_gather_records<<<grid_for(c, ((size_t)n + 31) / 32, GATHER_WARPS, per_sm), GATHER_WARPS * 32, 0, c->stream>>>(
                 n, perm2, w.spare, o7, perm_out);
             CK_LAUNCH();
             c->launches += 7;

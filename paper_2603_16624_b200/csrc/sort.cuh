@@ -216,16 +216,19 @@ constexpr int SORT_STAGE_THREADS = 256;
 constexpr int SORT_PER_THREAD = SORT_TILE / SORT_STAGE_THREADS;
 constexpr size_t SORT_STAGE_SMEM = (size_t)SORT_TILE * (8 * sizeof(double) + sizeof(uint32_t)) + 3 * SORT_MAX_BUCKETS * sizeof(uint32_t);   // 72.7 KB: 3 CTAs per SM
 
-// dest (in place of rank) and the per-(bucket, tile) histogram H[b * tiles + tile]
-__global__ void __launch_bounds__(256)
+// dest (in place of rank), the per-(tile, bucket) histogram H[tile][b] and its tile-local exclusive scan T[tile][b]
+// (where bucket b starts in the tile's bucket order); rows of SORT_MAX_BUCKETS entries, one CTA per tile
+__global__ void __launch_bounds__(SORT_MAX_BUCKETS)
 k_dest_and_tile_hist(uint32_t n, const int32_t* __restrict__ cell, uint32_t* __restrict__ rank_to_dest,
-                     const uint32_t* __restrict__ start, int shift, uint32_t tiles, uint32_t* __restrict__ H)
+                     const uint32_t* __restrict__ start, int shift, uint32_t* __restrict__ H, uint32_t* __restrict__ T)
 {
     __shared__ uint32_t cnt[SORT_MAX_BUCKETS];
-    for (int t = threadIdx.x; t < SORT_MAX_BUCKETS; t += blockDim.x) cnt[t] = 0;
+    __shared__ uint32_t total;
+    cnt[threadIdx.x] = 0;
     __syncthreads();
     const size_t p0 = (size_t)blockIdx.x * SORT_TILE;
-    for (int e = threadIdx.x; e < SORT_TILE; e += blockDim.x) {
+#pragma unroll
+    for (int e = threadIdx.x; e < SORT_TILE; e += SORT_MAX_BUCKETS) {
         const size_t p = p0 + e;
         if (p < n) {
             const uint32_t d = start[cell[p]] + rank_to_dest[p];
@@ -234,18 +237,61 @@ k_dest_and_tile_hist(uint32_t n, const int32_t* __restrict__ cell, uint32_t* __r
         }
     }
     __syncthreads();
-    const uint32_t nb = ((n - 1) >> shift) + 1;
-    for (uint32_t b = threadIdx.x; b < nb; b += blockDim.x) H[(size_t)b * tiles + blockIdx.x] = cnt[b];
+    const uint32_t c = cnt[threadIdx.x];
+    const uint32_t ex = block_exclusive_scan(c, &total);
+    const size_t row = (size_t)blockIdx.x * SORT_MAX_BUCKETS + threadIdx.x;
+    H[row] = c;
+    T[row] = ex;
+}
+
+// First slot of every (tile, bucket) share: Hs[tile][b] = (b << shift) + sum of H[t][b] over the tiles t < tile (every
+// bucket holds exactly 2^shift places).  Column-wise running sums, thread = bucket, in chunks of SORT_CHUNK tiles:
+// column sums per chunk, their running sums over the chunks, then the rows of every chunk.
+constexpr int SORT_CHUNK = 128;
+__global__ void __launch_bounds__(SORT_MAX_BUCKETS)
+k_tile_colsum(uint32_t tiles, const uint32_t* __restrict__ H, uint32_t* __restrict__ S)
+{
+    const uint32_t t0 = blockIdx.x * SORT_CHUNK, t1 = min(t0 + (uint32_t)SORT_CHUNK, tiles);
+    uint32_t sum = 0;
+    for (uint32_t t = t0; t < t1; ++t) sum += H[(size_t)t * SORT_MAX_BUCKETS + threadIdx.x];
+    S[(size_t)blockIdx.x * SORT_MAX_BUCKETS + threadIdx.x] = sum;
+}
+
+__global__ void __launch_bounds__(SORT_MAX_BUCKETS)
+k_tile_chunkscan(uint32_t chunks, uint32_t* __restrict__ S)
+{
+    uint32_t run = 0;
+    for (uint32_t ch = 0; ch < chunks; ++ch) {
+        const size_t i = (size_t)ch * SORT_MAX_BUCKETS + threadIdx.x;
+        const uint32_t v = S[i];
+        S[i] = run;
+        run += v;
+    }
+}
+
+__global__ void __launch_bounds__(SORT_MAX_BUCKETS)
+k_tile_colscan(uint32_t tiles, int shift, const uint32_t* __restrict__ H, const uint32_t* __restrict__ S,
+               uint32_t* __restrict__ Hs)
+{
+    const uint32_t t0 = blockIdx.x * SORT_CHUNK, t1 = min(t0 + (uint32_t)SORT_CHUNK, tiles);
+    uint32_t run = (threadIdx.x << shift) + S[(size_t)blockIdx.x * SORT_MAX_BUCKETS + threadIdx.x];
+    for (uint32_t t = t0; t < t1; ++t) {
+        const size_t i = (size_t)t * SORT_MAX_BUCKETS + threadIdx.x;
+        const uint32_t v = H[i];
+        Hs[i] = run;
+        run += v;
+    }
 }
 
 struct Sort7 { const double* in[7]; };
 
-// step A: the records of one tile.  H: per-(bucket, tile) histogram, Hs: its exclusive scan.  In shared memory word k of
-// the record at tile position lp sits at lp*8 + (k ^ (lp & 7)): the writes of a warp (one k, scattered lp) spread over
-// the banks, the 16-byte reads of the store phase stay aligned pairs (swapped where lp is odd).
+// step A: the records of one tile.  T: where bucket b starts in the tile's bucket order, Hs: the first slot of the tile's
+// share of bucket b.  In shared memory word k of the record at tile position lp sits at lp*8 + (k ^ (lp & 7)): the writes
+// of a warp (one k, scattered lp) spread over the banks, the 16-byte reads of the store phase stay aligned pairs (swapped
+// where lp is odd).
 __global__ void __launch_bounds__(SORT_STAGE_THREADS, 3)
-k_stage_records(uint32_t n, const uint32_t* __restrict__ dest, const uint32_t* __restrict__ H,
-                const uint32_t* __restrict__ Hs, int shift, uint32_t tiles, Sort7 a, double* __restrict__ tmp,
+k_stage_records(uint32_t n, const uint32_t* __restrict__ dest, const uint32_t* __restrict__ T,
+                const uint32_t* __restrict__ Hs, int shift, Sort7 a, double* __restrict__ tmp,
                 uint32_t* __restrict__ tmpdest)
 {
     extern __shared__ __align__(16) unsigned char stage_smem[];
@@ -254,18 +300,13 @@ k_stage_records(uint32_t n, const uint32_t* __restrict__ dest, const uint32_t* _
     uint32_t* base = slot + SORT_TILE;          // first slot of this tile's share of bucket b
     uint32_t* toff = base + SORT_MAX_BUCKETS;   // where bucket b starts in the tile's bucket order
     uint32_t* cnt = toff + SORT_MAX_BUCKETS;    // arrivals so far
-    __shared__ uint32_t total;
-    static_assert(SORT_MAX_BUCKETS <= SORT_STAGE_THREADS, "one thread per bucket in the tile-local scan");
-    const uint32_t nb = ((n - 1) >> shift) + 1;
-    const uint32_t b = threadIdx.x;
-    const uint32_t c = b < nb ? H[(size_t)b * tiles + blockIdx.x] : 0u;
-    const uint32_t ex = block_exclusive_scan(c, &total);
-    if (b < (uint32_t)SORT_MAX_BUCKETS) {
-        toff[b] = ex;
-        base[b] = b < nb ? Hs[(size_t)b * tiles + blockIdx.x] : 0u;
-        cnt[b] = 0u;
+    static_assert(SORT_MAX_BUCKETS == SORT_STAGE_THREADS, "one thread per bucket");
+    {
+        const size_t row = (size_t)blockIdx.x * SORT_MAX_BUCKETS + threadIdx.x;
+        toff[threadIdx.x] = T[row];
+        base[threadIdx.x] = Hs[row];
+        cnt[threadIdx.x] = 0u;
     }
-    __syncthreads();
     const size_t p0 = (size_t)blockIdx.x * SORT_TILE;
     const uint32_t tile_n = (uint32_t)min((size_t)SORT_TILE, (size_t)n - p0);
     // load phase: all 7 x SORT_PER_THREAD values of this thread are requested before the first is used
@@ -280,6 +321,7 @@ k_stage_records(uint32_t n, const uint32_t* __restrict__ dest, const uint32_t* _
             for (int k = 0; k < 7; ++k) v[j][k] = a.in[k][p0 + e];
         }
     }
+    __syncthreads();
 #pragma unroll
     for (int j = 0; j < SORT_PER_THREAD; ++j) {
         const uint32_t e = threadIdx.x + j * SORT_STAGE_THREADS;
