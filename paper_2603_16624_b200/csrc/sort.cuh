@@ -23,7 +23,7 @@ __device__ __forceinline__ int cell_of(const Geom& g, double x, double y, double
 // One thread per particle, HIST_ILP particles per thread and loop pass.  Lanes of a warp that fall in the same cell are
 // aggregated with match_any so that a cell-sorted input costs one atomic per (warp, cell) instead of 32; for an input
 // in arbitrary order every particle pays its own L2 atomic, whose round trip bounds the kernel: the HIST_ILP atomics of
-// a pass are issued before the first result is used.
+// a pass are issued before the first result is used (33.5 M random particles: 1 per pass 0.52 ms, 4: 0.43, 8: 0.56).
 constexpr int HIST_ILP = 4;
 template <bool WITH_RANK>
 __global__ void __launch_bounds__(256)
