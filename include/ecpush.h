@@ -82,7 +82,8 @@ int ecsim_init_grid(ecsim_ctx **ctx, int nx, int ny, int nz, double dx, double d
                     int n_species, void *cuda_stream);
 
 /* Scratch bytes needed for species holding at most n_particles_max particles each: per-species cell segment
- * tables, sort keys / ranks / permutation, seven spare arrays for the out-of-place permutation, stray lists,
+ * tables, sort keys / ranks / permutation, eight spare arrays for the out-of-place permutation (seven arrays of a
+ * re-sort, or the 64-byte records of a sort of arbitrary order), stray lists,
  * and the per-cell accumulator arrays AM[cells][244], AJ[n_species][cells][8][4] of the fused kernel. */
 size_t ecsim_workspace_bytes(const ecsim_ctx *ctx, int64_t n_particles_max);
 
