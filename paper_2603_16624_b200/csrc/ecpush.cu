@@ -516,12 +516,18 @@ extern "C" int ecsim_sort_particles(ecsim_ctx* c, int s, int32_t* cell_count_out
             CK_LAUNCH();
             k_invert_slots<<<grid, 256, 0, c->stream>>>(n, tmpdest, perm2);
             CK_LAUNCH();
-            // the places in flight (one per thread) must span less than one bucket, or the second record of a 128-byte
-            // line arrives after the line has left L2 (measured at 33.5 M particles, buckets of 131,072 places: 3 CTAs per
-            // SM 0.70 ms and 2.28 GB read, 4 per SM 0.94 ms and 3.08 GB); whole multiples of the SM count keep the CTAs abreast
+            // The two records of a 128-byte line are wanted at unrelated moments while their bucket is in flight: the bytes
+            // that pass through L2 in between -- (places of a bucket + places in flight, one per thread) x 120 B -- must stay
+            // well inside L2, or the line is fetched twice.  Measured at 33.5 M particles (buckets of 131,072 places): 3 CTAs
+            // per SM 0.69 ms and 2.28 GB read, 2 per SM 0.84 ms (too few loads in flight), 4 per SM 0.94 ms and 3.08 GB, 8 per
+            // SM 0.84 ms and 3.24 GB; whole multiples of the SM count keep the CTAs abreast.  Buckets too large for that
+            // rule (species above ~60 M particles in arbitrary order) run with full occupancy and pay the second fetch.
             int per_sm = 8;
-            if ((size_t)n * 64 > ((size_t)48 << 20))
-                per_sm = (int)std::min<size_t>(8, std::max<size_t>(1, ((size_t)9 << shift) / 10 / (GATHER_WARPS * 32) / (size_t)c->sm_count));
+            {
+                const size_t budget = ((size_t)32 << 20) / 120, bucket = (size_t)1 << shift;
+                const size_t fit = budget > bucket ? (budget - bucket) / (GATHER_WARPS * 32) / (size_t)c->sm_count : 0;
+                if (fit >= 2) per_sm = (int)std::min<size_t>(8, fit);
+            }
             k_gather_records<<<grid_for(c, ((size_t)n + 31) / 32, GATHER_WARPS, per_sm), GATHER_WARPS * 32, 0, c->stream>>>(
                 n, perm2, w.spare, o7, perm_out);
             CK_LAUNCH();

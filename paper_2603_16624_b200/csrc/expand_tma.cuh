@@ -53,10 +53,11 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity)
         "DONE_%=:\n"
         "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, uint64_t* bar)
+// (with an L2 evict-last policy: a cell's class sums are read by the four node columns around it, at different moments)
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, uint64_t* bar, unsigned long long pol)
 {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(pol) : "memory");
 }
 
 struct ExpandStreamArgs {
@@ -118,6 +119,8 @@ k_expand_M_stream(const __grid_constant__ ExpandStreamArgs a)
                                a.AM + ((size_t)i * g.ny + jm1) * g.nz * AM_PER_CELL,
                                a.AM + ((size_t)im1 * g.ny + j) * g.nz * AM_PER_CELL,
                                a.AM + ((size_t)im1 * g.ny + jm1) * g.nz * AM_PER_CELL};
+    unsigned long long keep;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(keep));
     auto issue = [&](int q) {      // thread 0 only
         if (q >= n_stages) return;
         const int z = q ? q - 1 : g.nz - 1;
@@ -127,7 +130,7 @@ k_expand_M_stream(const __grid_constant__ ExpandStreamArgs a)
 #pragma unroll
         for (int c = 0; c < 4; ++c)
             bulk_g2s(ring + (size_t)slot * XS_STAGE_DOUBLES + c * AM_PER_CELL, colsrc[c] + (size_t)z * AM_PER_CELL,
-                     AM_PER_CELL * 8, bar);
+                     AM_PER_CELL * 8, bar, keep);
     };
 
     if (tid == 0) {
@@ -199,7 +202,7 @@ k_expand_M_stream(const __grid_constant__ ExpandStreamArgs a)
                     else if (wxy[m] == 2) s = xs_sum<2, false>(s, offA, offB, off[m], nxy[m], two[m]);
                     else s = xs_sum<1, false>(s, offA, offB, off[m], nxy[m], two[m]);
                 }
-                *mptr[m] = s;
+                __stcs(mptr[m], s);                        // M is written once and not read here: streamed
             }
             mptr[m] += NOUT;
         }
