@@ -69,6 +69,51 @@ def test_cell_index_and_counting_sort_are_bit_exact(case):
     ctx.close()
 
 
+@pytest.mark.parametrize("n,dims", [(1, (3, 4, 5)), (31, (3, 4, 5)), (1024, (5, 7, 3)), (1025, (5, 7, 3)), (2047, (16, 9, 11)),
+                                    (8193, (2, 2, 2)), (300001, (40, 33, 21)), (2500000, (24, 20, 28))])
+@pytest.mark.parametrize("want_perm", [True, False], ids=["perm", "noperm"])
+def test_sort_of_arbitrary_order_tile_and_bucket_tails(n, dims, want_perm):
+    """The record-based two-step move (sort.cuh) at sizes around its tile (1024 records) and bucket (2^shift places)
+    boundaries: one ragged tile, several buckets with a partial last one, dense and sparse cells, with and without the
+    permutation output; then a second sort of the now sorted species (the near-identity path)."""
+    rng = np.random.default_rng(n)
+    grid = (*dims, 0.5, 1.25, 2.0)
+    cells = dims[0] * dims[1] * dims[2]
+    pn = rand_particles(rng, n, grid)
+    cell_ref, count_ref = oracle.cells(grid, pn["x"], pn["y"], pn["z"])
+    ctx = pk.Ecsim(*grid, 1)
+    ctx.set_workspace(n)
+    pc = {k: torch.from_numpy(pn[k]).cuda() for k in PKEYS}
+    ctx.load_particles(0, -3.0, pc, sorted=False)
+    count = torch.empty(cells, dtype=torch.int32, device="cuda")
+    perm = torch.empty(n, dtype=torch.int32, device="cuda") if want_perm else None
+    ctx.sort_particles(0, count, perm)
+    torch.cuda.synchronize()
+    assert np.array_equal(count.cpu().numpy(), count_ref)
+    got = {k: pc[k].cpu().numpy() for k in PKEYS}
+    if want_perm:
+        pm = perm.cpu().numpy().astype(np.int64) & 0xFFFFFFFF
+        assert np.array_equal(np.sort(pm), np.arange(n))
+        for k in PKEYS:
+            assert np.array_equal(got[k], pn[k][pm]), k
+    else:
+        # without the permutation: the multiset of particles is unchanged (q carries distinct random values)
+        order_in, order_out = np.argsort(pn["q"], kind="stable"), np.argsort(got["q"], kind="stable")
+        for k in PKEYS:
+            assert np.array_equal(got[k][order_out], pn[k][order_in]), k
+    cell_sorted, _ = oracle.cells(grid, got["x"], got["y"], got["z"])
+    assert np.all(np.diff(cell_sorted) >= 0)
+    # a second sort moves nothing across cells and keeps every particle
+    ctx.sort_particles(0, count, None)
+    torch.cuda.synchronize()
+    assert np.array_equal(count.cpu().numpy(), count_ref)
+    again = {k: pc[k].cpu().numpy() for k in PKEYS}
+    cell_again, _ = oracle.cells(grid, again["x"], again["y"], again["z"])
+    assert np.array_equal(cell_again, cell_sorted)
+    assert np.array_equal(np.sort(again["q"]), np.sort(pn["q"]))
+    ctx.close()
+
+
 # ------------------------------------------------------------------ the hot path, all five configs
 
 @pytest.mark.parametrize("variant", [pk.VARIANT_FUSED, pk.VARIANT_ATOMIC], ids=["fused", "atomic"])
