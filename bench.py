@@ -77,6 +77,7 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--cpu-sample-planes", type=int, default=8, help="x-planes of cells the oracle sample covers")
+    ap.add_argument("--no-rows", action="store_true", help="skip the timings of the separate SURVEY 8(f) calls (moments, push, apply_M, diagnostics)")
     ap.add_argument("--sustained-steps", type=int, default=-1,
                     help="consecutive steps WITHOUT restoring the particle state (default: 10; configs[1]: its 1 + 10 protocol; 0 = skip)")
     return ap.parse_args()
@@ -365,6 +366,7 @@ def run_product(args):
 
     # ---- what a time loop sees: the step WITH the segment-table build, and consecutive steps ----
     line["step_with_segments_ms"] = measure_with_segments(args, cfg, ctx, restore_arrays, one_step, world)
+    line["rows"] = None if args.no_rows else measure_rows(args, cfg, ctx, restore, E, B, rho, J, M, world)
     n_sus = args.sustained_steps if args.sustained_steps >= 0 else (cfg.steps if cfg.steps > 1 else 10)
     if n_sus > 0:
         line["sustained"] = measure_sustained(args, cfg, ctx, restore_arrays, work, E, B, rho, J, M, n_sus, n_total, world)
@@ -415,6 +417,45 @@ def measure_with_segments(args, cfg, ctx, restore_arrays, one_step, world):
         torch.cuda.synchronize()
         ms.append(e0.elapsed_time(e1))
     return max_over_ranks([_median(ms)], world)[0]
+
+
+def measure_rows(args, cfg, ctx, restore, E, B, rho, J, M, world):
+    """The other entry points of SURVEY 8(f) on the same workload, from the sorted state, CUDA events, median of 3:
+    the two halves of a real time step (ecsim_moments_all, ecsim_push_all), the operator sum M E (ecsim_apply_M; HBM-bound:
+    its GB/s count M read once + E + out) and the diagnostic moments of species 0 (ecsim_diagnostics)."""
+    import torch
+    import paper_2603_16624_b200 as pk
+    dev = E.device
+    nodes = cfg.nodes
+
+    def timed(fn, prepare=None):
+        ms = []
+        for _ in range(3):
+            if prepare:
+                prepare()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); fn(); e1.record()
+            torch.cuda.synchronize()
+            ms.append(e0.elapsed_time(e1))
+        return max_over_ranks([_median(ms)], world)[0]
+
+    out = {}
+    restore()
+    out["moments_all_ms"] = timed(lambda: ctx.moments_all(B, cfg.dt, rho, J, M, accumulate=pk.ACC_NONE))
+    out["push_all_ms"] = timed(lambda: ctx.push_all(E, B, cfg.dt, cfg.theta), prepare=restore)
+    restore()
+    ctx.moments_all(B, cfg.dt, rho, J, M, accumulate=pk.ACC_NONE)
+    ME = torch.empty(3, nodes, dtype=torch.float64, device=dev)
+    t = timed(lambda: ctx.apply_M(M, E, ME))
+    out["apply_M_ms"] = t
+    out["apply_M_GBps"] = (M.numel() + 6 * nodes) * 8 / (t * 1e-3) / 1e9
+    d_rho = torch.empty(nodes, dtype=torch.float64, device=dev)
+    d_J = torch.empty(3, nodes, dtype=torch.float64, device=dev)
+    d_P = torch.empty(6, nodes, dtype=torch.float64, device=dev)
+    d_Q = torch.empty(3, nodes, dtype=torch.float64, device=dev)
+    out["diagnostics_species0_ms"] = timed(lambda: ctx.diagnostics(0, d_rho, d_J, d_P, d_Q))
+    return out
 
 
 def measure_sustained(args, cfg, ctx, restore_arrays, work, E, B, rho, J, M, n_steps, n_total, world):

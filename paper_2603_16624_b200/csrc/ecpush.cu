@@ -1256,7 +1256,8 @@ extern "C" int ecsim_apply_M(ecsim_ctx* c, const double* M, const double* E, dou
 {
     if (!c || !M || !E || !out || E == out) return ECSIM_ERR_INVALID_ARG;
     ApplyMArgs a{c->g, M, E, out, accumulate ? 1 : 0};
-    const size_t blocks_needed = ((size_t)c->g.nodes + APPLY_WARPS - 1) / APPLY_WARPS;
+    const size_t runs = (size_t)c->g.nx * c->g.ny * (size_t)((c->g.nz + APPLY_RUN - 1) / APPLY_RUN);
+    const size_t blocks_needed = (runs + APPLY_WARPS - 1) / APPLY_WARPS;
     size_t grid = (size_t)c->sm_count * 8;
     if (grid > blocks_needed) grid = blocks_needed;
     if (c->m_layout == ECSIM_M_14) k_apply_M<14><<<(int)grid, APPLY_WARPS * 32, 0, c->stream>>>(a);
