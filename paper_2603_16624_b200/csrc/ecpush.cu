@@ -907,7 +907,7 @@ static cudaError_t launch_fused_any(const ecsim_ctx* c, const FusedArgs& fa, int
     if (mode == MODE_DIAG)
         return gapped ? launch_fused<16, 128, MODE_DIAG, LAYOUT_GAPPED>(c, fa) : launch_fused<16, 128, MODE_DIAG, LAYOUT_DENSE>(c, fa);
     if (mode == MODE_PUSH)
-        return gapped ? launch_fused<16, 128, MODE_PUSH, LAYOUT_GAPPED>(c, fa) : launch_fused<16, 128, MODE_PUSH, LAYOUT_DENSE>(c, fa);
+        return gapped ? launch_fused<16, 128, MODE_PUSH, LAYOUT_GAPPED>(c, fa) : launch_fused<20, 96, MODE_PUSH, LAYOUT_DENSE>(c, fa);
     if (mode == MODE_MOMENTS)
         return gapped ? launch_fused<12, 168, MODE_MOMENTS, LAYOUT_GAPPED>(c, fa) : launch_fused<12, 168, MODE_MOMENTS, LAYOUT_DENSE>(c, fa);
     if (gapped) return launch_fused<12, 168, MODE_FUSED, LAYOUT_GAPPED>(c, fa);

@@ -513,6 +513,12 @@ k_fused_push_moments(const __grid_constant__ FusedArgs a)
                 }
             }
 
+            // push only: there is no phase 2 for the next batch's loads to fly under, and registers to spare, so they are
+            // requested before phase 1 (config 2, ecsim_push_all: 16 warps x 128 registers 6.0 ms; with the early loads 5.64; 20 x 96
+            // with them 5.33 = 5.2 TB/s; 24 x 80 and 32 x 64 spill: 6.2 / 6.5; no gain for the diagnostics)
+            constexpr bool EARLY_FETCH = MODE == MODE_PUSH;
+            if (EARLY_FETCH && (in_state == 1 || in_state == 2)) fetch();
+
             // ---- phase 1: lane = particle ----
             PushedRegs o;
             const bool active = lane < nb;
@@ -538,7 +544,7 @@ k_fused_push_moments(const __grid_constant__ FusedArgs a)
             }
             // global loads of the next batch fly during phase 2 (requesting them before phase 1 was measured: 11.90 vs
             // 11.65 ms, the 14 extra live registers cost more than the longer flight time gains)
-            if (in_state == 1 || in_state == 2) fetch();
+            if (!EARLY_FETCH && (in_state == 1 || in_state == 2)) fetch();
             if (in_state != 1 && has_next) { load_fields(ni, nj, nk, f0, f1); fld_ready = true; }
             if (!GAPPED) {
                 const unsigned smask = __ballot_sync(0xffffffffu, active && !inside);
