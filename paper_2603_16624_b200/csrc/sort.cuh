@@ -286,9 +286,7 @@ k_tile_colscan(uint32_t tiles, int shift, const uint32_t* __restrict__ H, const 
 struct Sort7 { const double* in[7]; };
 
 // step A: the records of one tile.  T: where bucket b starts in the tile's bucket order, Hs: the first slot of the tile's
-// share of bucket b.  In shared memory word k of the record at tile position lp sits at lp*8 + (k ^ (lp & 7)): the writes
-// of a warp (one k, scattered lp) spread over the banks, the 16-byte reads of the store phase stay aligned pairs (swapped
-// where lp is odd).
+// share of bucket b.
 __global__ void __launch_bounds__(SORT_STAGE_THREADS, 3)
 k_stage_records(uint32_t n, const uint32_t* __restrict__ dest, const uint32_t* __restrict__ T,
                 const uint32_t* __restrict__ Hs, int shift, Sort7 a, double* __restrict__ tmp,
@@ -330,24 +328,26 @@ k_stage_records(uint32_t n, const uint32_t* __restrict__ dest, const uint32_t* _
             const uint32_t r = atomicAdd(&cnt[bk], 1u);
             const uint32_t lp = toff[bk] + r;
             slot[lp] = base[bk] + r;
-            double* w = rec + (size_t)lp * 8;
-            const uint32_t sw = lp & 7u;
-#pragma unroll
-            for (int k = 0; k < 7; ++k) w[k ^ sw] = v[j][k];
+            // 16-byte piece p of the record at tile position lp sits at piece p ^ ((lp >> 1) & 3): the four STS.128 of a warp
+            // (one piece each, scattered lp) spread over all eight 16-byte bank groups
+            double2* w = reinterpret_cast<double2*>(rec + (size_t)lp * 8);
+            const uint32_t sw = (lp >> 1) & 3u;
+            w[0u ^ sw] = make_double2(v[j][0], v[j][1]);
+            w[1u ^ sw] = make_double2(v[j][2], v[j][3]);
+            w[2u ^ sw] = make_double2(v[j][4], v[j][5]);
             // the original index (low word) and the final place (high word) travel with the record
-            w[7 ^ sw] = __longlong_as_double((long long)(((unsigned long long)d[j] << 32) | (unsigned long long)(p0 + e)));
+            w[3u ^ sw] = make_double2(v[j][6], __longlong_as_double((long long)(((unsigned long long)d[j] << 32) | (unsigned long long)(p0 + e))));
         }
     }
     __syncthreads();
     // store phase: 16-byte pieces, consecutive threads = consecutive pieces of consecutive records of a run
     for (uint32_t t = threadIdx.x; t < tile_n * 4u; t += SORT_STAGE_THREADS) {
-        const uint32_t r = t >> 2, part = t & 3u, sw = r & 7u;
-        double2 pr = *reinterpret_cast<const double2*>(rec + (size_t)r * 8 + ((2u * part) ^ (sw & 6u)));
-        if (sw & 1u) { const double h = pr.x; pr.x = pr.y; pr.y = h; }
+        const uint32_t r = t >> 2, part = t & 3u;
+        const double2 pr = *reinterpret_cast<const double2*>(rec + (size_t)r * 8 + 2u * (part ^ ((r >> 1) & 3u)));
         *reinterpret_cast<double2*>(tmp + (size_t)slot[r] * 8 + 2u * part) = pr;
     }
     for (uint32_t t = threadIdx.x; t < tile_n; t += SORT_STAGE_THREADS)
-        tmpdest[slot[t]] = (uint32_t)((unsigned long long)__double_as_longlong(rec[(size_t)t * 8 + (7u ^ (t & 7u))]) >> 32);
+        tmpdest[slot[t]] = (uint32_t)((unsigned long long)__double_as_longlong(rec[(size_t)t * 8 + 2u * (3u ^ ((t >> 1) & 3u)) + 1u]) >> 32);
 }
 
 struct Move7 { const double* src[7]; double* dst[7]; };
