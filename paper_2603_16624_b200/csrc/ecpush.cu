@@ -514,7 +514,14 @@ extern "C" int ecsim_sort_particles(ecsim_ctx* c, int s, int32_t* cell_count_out
             k_stage_records<<<tiles, SORT_STAGE_THREADS, SORT_STAGE_SMEM, c->stream>>>(n, dest, T, w.tile_scan, shift, s7, w.spare,
                                                                                     tmpdest);
             CK_LAUNCH();
-            k_invert_slots<<<grid, 256, 0, c->stream>>>(n, tmpdest, perm2);
+            if (((uint32_t)1 << shift) <= 4u * (uint32_t)INV_SUB) {
+                const uint32_t sub = std::min<uint32_t>((uint32_t)1 << shift, (uint32_t)INV_SUB), per_bucket = ((uint32_t)1 << shift) / sub;
+                const uint32_t nbk = ((n - 1) >> shift) + 1;
+                CK(cudaFuncSetAttribute(k_invert_slots_local, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(INV_SUB * sizeof(uint32_t))));
+                k_invert_slots_local<<<nbk * per_bucket, INV_THREADS, sub * sizeof(uint32_t), c->stream>>>(n, shift, tmpdest, perm2);
+            } else {
+                k_invert_slots<<<grid, 256, 0, c->stream>>>(n, tmpdest, perm2);
+            }
             CK_LAUNCH();
             // The two records of a 128-byte line are wanted at unrelated moments while their bucket is in flight: the bytes
             // that pass through L2 in between -- (places of a bucket + places in flight, one per thread) x 120 B -- must stay

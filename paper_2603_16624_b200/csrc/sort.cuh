@@ -201,7 +201,7 @@ k_copy_u32_to_i32(uint32_t m, const uint32_t* __restrict__ in, int32_t* __restri
 //   step A, k_stage_records: a tile of SORT_TILE particles per CTA.  A particle's slot = (places of its bucket taken
 //          by earlier tiles, from the scanned per-(bucket, tile) histogram) + (its arrival rank in the tile, a shared-
 //          memory atomic).  The seven values of a particle are read once (coalesced SoA loads, 28 in flight per
-//          thread), put together as ONE 64-byte record {x,y,z,u,v,w,q, (dest, original index)} at the particle's position in
+//          thread at 1024, 14 at 512), put together as ONE 64-byte record {x,y,z,u,v,w,q, (dest, original index)} at the particle's position in
 //          the tile's bucket order in shared memory, and the tile is written to tmp[] in runs of ~SORT_TILE/buckets
 //          whole records: one load phase, one barrier, one store phase per tile (round 2 first moved array by array:
 //          seven load / store phase pairs per tile, 128-byte runs, 1.52 ms per 33.5 M particles at 2.9 TB/s).
@@ -209,12 +209,13 @@ k_copy_u32_to_i32(uint32_t m, const uint32_t* __restrict__ in, int32_t* __restri
 //          one record (two whole sectors; the 8-byte gather of the SoA version fetched seven sectors per particle and
 //          ran at 83 % of the L1 tag rate, ncu), a per-warp transposition in shared memory, seven coalesced stores.
 //          The sources of the places in flight lie inside the windows of a few buckets (2^shift records of 64 B).
-// tmp = eight spare arrays of the workspace.
-constexpr int SORT_TILE = 1024;
+// tmp = eight spare arrays of the workspace.  Tile size, 33.5 M particles, step A + table kernels: 1024 records (3 CTAs
+// per SM) 0.89 + 0.22 ms, 512 (5 CTAs) 0.76 + 0.27, 256 (8 CTAs) 0.85 + 0.38.
+constexpr int SORT_TILE = 512;
 constexpr int SORT_MAX_BUCKETS = 256;
 constexpr int SORT_STAGE_THREADS = 256;
 constexpr int SORT_PER_THREAD = SORT_TILE / SORT_STAGE_THREADS;
-constexpr size_t SORT_STAGE_SMEM = (size_t)SORT_TILE * (8 * sizeof(double) + sizeof(uint32_t)) + 3 * SORT_MAX_BUCKETS * sizeof(uint32_t);   // 72.7 KB: 3 CTAs per SM
+constexpr size_t SORT_STAGE_SMEM = (size_t)SORT_TILE * (8 * sizeof(double) + sizeof(uint32_t)) + 3 * SORT_MAX_BUCKETS * sizeof(uint32_t);   // 37.9 KB: 5 CTAs per SM
 
 // dest (in place of rank), the per-(tile, bucket) histogram H[tile][b] and its tile-local exclusive scan T[tile][b]
 // (where bucket b starts in the tile's bucket order); rows of SORT_MAX_BUCKETS entries, one CTA per tile
@@ -287,7 +288,7 @@ struct Sort7 { const double* in[7]; };
 
 // step A: the records of one tile.  T: where bucket b starts in the tile's bucket order, Hs: the first slot of the tile's
 // share of bucket b.
-__global__ void __launch_bounds__(SORT_STAGE_THREADS, 3)
+__global__ void __launch_bounds__(SORT_STAGE_THREADS, 5)
 k_stage_records(uint32_t n, const uint32_t* __restrict__ dest, const uint32_t* __restrict__ T,
                 const uint32_t* __restrict__ Hs, int shift, Sort7 a, double* __restrict__ tmp,
                 uint32_t* __restrict__ tmpdest)
@@ -360,6 +361,38 @@ k_invert_slots(uint32_t n, const uint32_t* __restrict__ tmpdest, uint32_t* __res
 {
     const size_t stride = (size_t)gridDim.x * blockDim.x;
     for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += stride) perm2[tmpdest[t]] = (uint32_t)t;
+}
+
+// The same inverse without the scattered global stores, for buckets of <= 4 x INV_SUB places: a CTA owns INV_SUB consecutive
+// places of one bucket, streams the bucket's tmpdest window (coalesced; the window's other CTAs read it from L2), keeps the
+// entries that point into its places in shared memory and writes its part of perm2 coalesced.  (33.5 M particles: 0.29 ms
+// as a scatter -- 117 G partial L2 writes per second -- against the time below.)
+constexpr int INV_SUB = 32768;
+constexpr int INV_THREADS = 1024;
+__global__ void __launch_bounds__(INV_THREADS)
+k_invert_slots_local(uint32_t n, int shift, const uint32_t* __restrict__ tmpdest, uint32_t* __restrict__ perm2)
+{
+    extern __shared__ uint32_t inv_smem[];
+    const uint32_t bucket_places = 1u << shift;
+    const uint32_t sub = min(bucket_places, (uint32_t)INV_SUB), subs_per_bucket = bucket_places / sub;
+    const uint32_t bucket = blockIdx.x / subs_per_bucket, part = blockIdx.x % subs_per_bucket;
+    const size_t b0 = (size_t)bucket << shift, b1 = min(b0 + bucket_places, (size_t)n);
+    const size_t lo = b0 + (size_t)part * sub;
+    if (lo >= b1) return;
+    const uint32_t len = (uint32_t)min((size_t)sub, b1 - lo);
+    for (size_t t0 = b0 + threadIdx.x; t0 < b1; t0 += 8 * INV_THREADS) {      // eight loads in flight per thread
+        uint32_t d[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const size_t t = t0 + (size_t)j * INV_THREADS;
+            d[j] = t < b1 ? __ldg(tmpdest + t) : 0xffffffffu;
+        }
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+            if (d[j] >= lo && d[j] - lo < len) inv_smem[d[j] - (uint32_t)lo] = (uint32_t)(t0 + (size_t)j * INV_THREADS);
+    }
+    __syncthreads();
+    for (uint32_t i = threadIdx.x; i < len; i += INV_THREADS) perm2[lo + i] = inv_smem[i];
 }
 
 struct Out7 { double* dst[7]; };
