@@ -2,7 +2,7 @@
 ("close the parity gap at full size"):
 
   * configs[4] (64^3, 2 x 33,554,432 particles in seeded RANDOM order): the bucketed two-step counting sort at
-    shift = 17, 256 buckets x 32768 tiles of 1024 records -- per-cell counts bit-exact against oracle.cells, perm a permutation, the
+    shift = 17, 256 buckets x 65536 tiles of 512 records -- per-cell counts bit-exact against oracle.cells, perm a permutation, the
     seven moved arrays equal in[perm] bit for bit, cells ascending -- then one all-species step compared with the
     oracle on sampled 3x3x3 blocks of cells (same sampling argument as test_gpu_fullsize.py);
   * configs[1] (32^3, 4,194,304 particles): the whole "one step, then 10 consecutive steps, fields fixed" protocol,
