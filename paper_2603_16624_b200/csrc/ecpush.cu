@@ -84,10 +84,10 @@ struct Workspace {
     uint32_t* perm = nullptr;        // [n_max]
     double* spare = nullptr;         // [8][n_max]: the seven arrays of a species on their way through a re-sort, or its
                                      // n_max 64-byte records on their way through a sort of arbitrary order
-    uint32_t* tile_hist = nullptr;   // [tiles][SORT_MAX_BUCKETS] of the two-step move of a random-order sort
+    uint32_t* tile_hist = nullptr;   // [tiles][NB] of the two-step move of a random-order sort
     uint32_t* tile_off = nullptr;    // its tile-local exclusive scans over the buckets
     uint32_t* tile_scan = nullptr;   // first slot of every (tile, bucket) share
-    uint32_t* tile_sums = nullptr;   // [chunks of tiles][SORT_MAX_BUCKETS] column sums
+    uint32_t* tile_sums = nullptr;   // [chunks of tiles][NB] column sums
     uint32_t* stray_list = nullptr;  // [n_species][n_max]
     double* AM = nullptr;            // [cells][AM_PER_CELL = 244]
     double* AJ = nullptr;            // [n_species][cells][32]
@@ -155,11 +155,11 @@ static size_t carve(const ecsim_ctx* c, int64_t n_max, void* base, Workspace* ou
     w.perm = k.take<uint32_t>(n);
     w.spare = k.take<double>(8 * n);
     {
-        const size_t m = (size_t)SORT_MAX_BUCKETS * (n / SORT_TILE + 1);
+        const size_t m = sort_table_entries(n);
         w.tile_hist = k.take<uint32_t>(m);
         w.tile_off = k.take<uint32_t>(m);
         w.tile_scan = k.take<uint32_t>(m + 1);
-        w.tile_sums = k.take<uint32_t>(((n / SORT_TILE + 1) / SORT_CHUNK + 1) * (size_t)SORT_MAX_BUCKETS);
+        w.tile_sums = k.take<uint32_t>(sort_chunk_entries(n));
     }
     w.stray_list = k.take<uint32_t>(nsp * n);
     w.AM = k.take<double>(cells * AM_PER_CELL);
@@ -455,6 +455,36 @@ extern "C" int ecsim_build_segments(ecsim_ctx* c, int s)
 
 static int resident_layout_from_dense(ecsim_ctx* c, int s, const double* const src[7], int dst_buf);
 
+// Step A of the sort of a species in arbitrary order (sort.cuh) in one of its two geometries: final places, per-tile bucket
+// tables, first slots, then the records of every tile into ws.spare.  *shift_out: log2 of the bucket size chosen.
+template <int NB, int TILE>
+static int stage_records(ecsim_ctx* c, uint32_t n, const uint32_t* start, uint32_t* dest, double* const arrays[7],
+                         uint32_t* tmpdest, int* shift_out)
+{
+    Workspace& w = c->ws;
+    const size_t smem = sort_stage_smem(NB, TILE);
+    CK(cudaFuncSetAttribute(k_stage_records<NB, TILE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int shift = 13;
+    while ((((n - 1) >> shift) + 1) > (uint32_t)NB) ++shift;
+    const uint32_t tiles = (n + TILE - 1) / TILE;
+    const uint32_t chunks = (tiles + SORT_CHUNK - 1) / SORT_CHUNK;
+    k_dest_and_tile_hist<NB, TILE><<<tiles, NB, 0, c->stream>>>(n, w.cell, dest, start, shift, w.tile_hist, w.tile_off);
+    CK_LAUNCH();
+    k_tile_colsum<<<chunks, NB, 0, c->stream>>>(tiles, w.tile_hist, w.tile_sums);
+    CK_LAUNCH();
+    k_tile_chunkscan<<<1, NB, 0, c->stream>>>(chunks, w.tile_sums);
+    CK_LAUNCH();
+    k_tile_colscan<<<chunks, NB, 0, c->stream>>>(tiles, shift, w.tile_hist, w.tile_sums, w.tile_scan);
+    CK_LAUNCH();
+    Sort7 s7;
+    for (int a = 0; a < 7; ++a) s7.in[a] = arrays[a];
+    k_stage_records<NB, TILE><<<tiles, NB, smem, c->stream>>>(n, dest, w.tile_off, w.tile_scan, shift, s7, w.spare, tmpdest);
+    CK_LAUNCH();
+    c->launches += 5;
+    *shift_out = shift;
+    return ECSIM_OK;
+}
+
 extern "C" int ecsim_sort_particles(ecsim_ctx* c, int s, int32_t* cell_count_out, uint32_t* perm_out)
 {
     int rc = check_species(c, s);
@@ -491,29 +521,16 @@ extern "C" int ecsim_sort_particles(ecsim_ctx* c, int s, int32_t* cell_count_out
                 CK(cudaMemcpyAsync(perm_out, w.perm, sizeof(uint32_t) * (size_t)n, cudaMemcpyDeviceToDevice, c->stream));
         } else {
             // arbitrary order: the bucketed two-step move of sort.cuh through 64-byte records
-            CK(cudaFuncSetAttribute(k_stage_records, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SORT_STAGE_SMEM));
-            int shift = 13;
-            while ((((n - 1) >> shift) + 1) > (uint32_t)SORT_MAX_BUCKETS) ++shift;
-            const uint32_t tiles = (n + SORT_TILE - 1) / SORT_TILE;
             uint32_t* dest = w.rank;                                   // rank -> dest in place
             uint32_t* tmpdest = w.perm;
+            int shift = 13;
+            rc = n <= SORT_SMALL_MAX_N   ? stage_records<SORT_NB_SMALL, SORT_TILE_SMALL>(c, n, start, dest, arrays, tmpdest, &shift)
+                 : n <= SORT_LARGE_MAX_N ? stage_records<SORT_NB_LARGE, SORT_TILE_LARGE>(c, n, start, dest, arrays, tmpdest, &shift)
+                                         : stage_records<SORT_NB_HUGE, SORT_TILE_HUGE>(c, n, start, dest, arrays, tmpdest, &shift);
+            if (rc) return rc;
             uint32_t* perm2 = w.stray_list + (size_t)s * (size_t)w.n_max;      // (the stray lists are idle during a sort)
-            uint32_t* T = w.tile_off;
-            const uint32_t chunks = (tiles + SORT_CHUNK - 1) / SORT_CHUNK;
-            k_dest_and_tile_hist<<<tiles, SORT_MAX_BUCKETS, 0, c->stream>>>(n, w.cell, dest, start, shift, w.tile_hist, T);
-            CK_LAUNCH();
-            k_tile_colsum<<<chunks, SORT_MAX_BUCKETS, 0, c->stream>>>(tiles, w.tile_hist, w.tile_sums);
-            CK_LAUNCH();
-            k_tile_chunkscan<<<1, SORT_MAX_BUCKETS, 0, c->stream>>>(chunks, w.tile_sums);
-            CK_LAUNCH();
-            k_tile_colscan<<<chunks, SORT_MAX_BUCKETS, 0, c->stream>>>(tiles, shift, w.tile_hist, w.tile_sums, w.tile_scan);
-            CK_LAUNCH();
-            Sort7 s7;
             Out7 o7;
-            for (int a = 0; a < 7; ++a) { s7.in[a] = arrays[a]; o7.dst[a] = arrays[a]; }
-            k_stage_records<<<tiles, SORT_STAGE_THREADS, SORT_STAGE_SMEM, c->stream>>>(n, dest, T, w.tile_scan, shift, s7, w.spare,
-                                                                                    tmpdest);
-            CK_LAUNCH();
+            for (int a = 0; a < 7; ++a) o7.dst[a] = arrays[a];
             if (((uint32_t)1 << shift) <= 4u * (uint32_t)INV_SUB) {
                 const uint32_t sub = std::min<uint32_t>((uint32_t)1 << shift, (uint32_t)INV_SUB), per_bucket = ((uint32_t)1 << shift) / sub;
                 const uint32_t nbk = ((n - 1) >> shift) + 1;
@@ -528,7 +545,7 @@ extern "C" int ecsim_sort_particles(ecsim_ctx* c, int s, int32_t* cell_count_out
             // well inside L2, or the line is fetched twice.  Measured at 33.5 M particles (buckets of 131,072 places): 3 CTAs
             // per SM 0.69 ms and 2.28 GB read, 2 per SM 0.84 ms (too few loads in flight), 4 per SM 0.94 ms and 3.08 GB, 8 per
             // SM 0.84 ms and 3.24 GB; whole multiples of the SM count keep the CTAs abreast.  Buckets too large for that
-            // rule (species above ~60 M particles in arbitrary order) run with full occupancy and pay the second fetch.
+            // rule (species above ~130 M particles in arbitrary order) run with full occupancy and pay the second fetch.
             int per_sm = 8;
             {
                 const size_t budget = ((size_t)32 << 20) / 120, bucket = (size_t)1 << shift;
@@ -538,7 +555,7 @@ extern "C" int ecsim_sort_particles(ecsim_ctx* c, int s, int32_t* cell_count_out
             k_gather_records<<<grid_for(c, ((size_t)n + 31) / 32, GATHER_WARPS, per_sm), GATHER_WARPS * 32, 0, c->stream>>>(
                 n, perm2, w.spare, o7, perm_out);
             CK_LAUNCH();
-            c->launches += 7;
+            c->launches += 2;
         }
     }
     if (cell_count_out) {

@@ -196,13 +196,13 @@ k_copy_u32_to_i32(uint32_t m, const uint32_t* __restrict__ in, int32_t* __restri
 // A random 8-byte gather from HBM costs ~97 bytes of traffic on B200 (3.26 GB per 33.5 M elements,
 // profiles/r01d), and scattered 8-byte stores are read-modify-writes of their sectors, so the permutation is
 // applied in two steps that are both local.  dest[p] = start[cell[p]] + rank[p] is the final place of particle p;
-// places are cut into <= SORT_MAX_BUCKETS buckets of 2^shift consecutive places (every bucket is full,
+// places are cut into <= NB buckets of 2^shift consecutive places (every bucket is full,
 // dest being a permutation).
-//   step A, k_stage_records: a tile of SORT_TILE particles per CTA.  A particle's slot = (places of its bucket taken
+//   step A, k_stage_records: a tile of TILE particles per CTA.  A particle's slot = (places of its bucket taken
 //          by earlier tiles, from the scanned per-(bucket, tile) histogram) + (its arrival rank in the tile, a shared-
 //          memory atomic).  The seven values of a particle are read once (coalesced SoA loads, 28 in flight per
 //          thread at 1024, 14 at 512), put together as ONE 64-byte record {x,y,z,u,v,w,q, (dest, original index)} at the particle's position in
-//          the tile's bucket order in shared memory, and the tile is written to tmp[] in runs of ~SORT_TILE/buckets
+//          the tile's bucket order in shared memory, and the tile is written to tmp[] in runs of ~TILE/buckets
 //          whole records: one load phase, one barrier, one store phase per tile (round 2 first moved array by array:
 //          seven load / store phase pairs per tile, 128-byte runs, 1.52 ms per 33.5 M particles at 2.9 TB/s).
 //   step B, k_invert_slots + k_gather_records: perm2 = tmpdest^-1, then place d takes record perm2[d]: four lanes read
@@ -211,25 +211,34 @@ k_copy_u32_to_i32(uint32_t m, const uint32_t* __restrict__ in, int32_t* __restri
 //          The sources of the places in flight lie inside the windows of a few buckets (2^shift records of 64 B).
 // tmp = eight spare arrays of the workspace.  Tile size, 33.5 M particles, step A + table kernels: 1024 records (3 CTAs
 // per SM) 0.89 + 0.22 ms, 512 (5 CTAs) 0.76 + 0.27, 256 (8 CTAs) 0.85 + 0.38.
-constexpr int SORT_TILE = 512;
-constexpr int SORT_MAX_BUCKETS = 256;
-constexpr int SORT_STAGE_THREADS = 256;
-constexpr int SORT_PER_THREAD = SORT_TILE / SORT_STAGE_THREADS;
-constexpr size_t SORT_STAGE_SMEM = (size_t)SORT_TILE * (8 * sizeof(double) + sizeof(uint32_t)) + 3 * SORT_MAX_BUCKETS * sizeof(uint32_t);   // 37.9 KB: 5 CTAs per SM
+// Three geometries <buckets NB = threads of a step-A CTA, TILE>, chosen by the species' size so that a bucket stays at
+// <= 131,072 places (step B's windows inside L2, the inverse built in shared memory): <256, 512> (5 CTAs per SM) up to 2^25
+// particles, <512, 1024> up to 2^26, <1024, 2048> above.  With the first geometry alone the sort cost 0.069 ns per particle
+// at 33.5 M particles but 0.085 / 0.092 / 0.105 at 50 / 67 / 134 M; with the three it stays at 0.070 - 0.072 (134 M: 9.7 ms).
+constexpr int SORT_NB_SMALL = 256, SORT_TILE_SMALL = 512;
+constexpr int SORT_NB_LARGE = 512, SORT_TILE_LARGE = 1024;
+constexpr int SORT_NB_HUGE = 1024, SORT_TILE_HUGE = 2048;
+constexpr uint32_t SORT_SMALL_MAX_N = 1u << 25, SORT_LARGE_MAX_N = 1u << 26;
+constexpr size_t sort_stage_smem(int nb, int tile) { return (size_t)tile * (8 * sizeof(double) + sizeof(uint32_t)) + 3 * (size_t)nb * sizeof(uint32_t); }
+// table entries (rows of NB per tile) and chunk sums for at most n particles, whichever geometry is used
+constexpr int SORT_CHUNK = 128;
+constexpr size_t sort_table_entries(size_t n) { return n / 2 + 2 * SORT_NB_HUGE; }
+constexpr size_t sort_chunk_entries(size_t n) { return n / 256 + 2 * SORT_NB_HUGE; }
 
 // dest (in place of rank), the per-(tile, bucket) histogram H[tile][b] and its tile-local exclusive scan T[tile][b]
-// (where bucket b starts in the tile's bucket order); rows of SORT_MAX_BUCKETS entries, one CTA per tile
-__global__ void __launch_bounds__(SORT_MAX_BUCKETS)
+// (where bucket b starts in the tile's bucket order); rows of NB entries, one CTA of NB threads per tile
+template <int NB, int TILE>
+__global__ void __launch_bounds__(NB)
 k_dest_and_tile_hist(uint32_t n, const int32_t* __restrict__ cell, uint32_t* __restrict__ rank_to_dest,
                      const uint32_t* __restrict__ start, int shift, uint32_t* __restrict__ H, uint32_t* __restrict__ T)
 {
-    __shared__ uint32_t cnt[SORT_MAX_BUCKETS];
+    __shared__ uint32_t cnt[NB];
     __shared__ uint32_t total;
     cnt[threadIdx.x] = 0;
     __syncthreads();
-    const size_t p0 = (size_t)blockIdx.x * SORT_TILE;
+    const size_t p0 = (size_t)blockIdx.x * TILE;
 #pragma unroll
-    for (int e = threadIdx.x; e < SORT_TILE; e += SORT_MAX_BUCKETS) {
+    for (int e = threadIdx.x; e < TILE; e += NB) {
         const size_t p = p0 + e;
         if (p < n) {
             const uint32_t d = start[cell[p]] + rank_to_dest[p];
@@ -240,44 +249,44 @@ k_dest_and_tile_hist(uint32_t n, const int32_t* __restrict__ cell, uint32_t* __r
     __syncthreads();
     const uint32_t c = cnt[threadIdx.x];
     const uint32_t ex = block_exclusive_scan(c, &total);
-    const size_t row = (size_t)blockIdx.x * SORT_MAX_BUCKETS + threadIdx.x;
+    const size_t row = (size_t)blockIdx.x * NB + threadIdx.x;
     H[row] = c;
     T[row] = ex;
 }
 
 // First slot of every (tile, bucket) share: Hs[tile][b] = (b << shift) + sum of H[t][b] over the tiles t < tile (every
-// bucket holds exactly 2^shift places).  Column-wise running sums, thread = bucket, in chunks of SORT_CHUNK tiles:
-// column sums per chunk, their running sums over the chunks, then the rows of every chunk.
-constexpr int SORT_CHUNK = 128;
-__global__ void __launch_bounds__(SORT_MAX_BUCKETS)
+// bucket holds exactly 2^shift places).  Column-wise running sums, thread = bucket (blockDim.x = NB = the row pitch), in
+// chunks of SORT_CHUNK tiles: column sums per chunk, their running sums over the chunks, then the rows of every chunk.
+__global__ void __launch_bounds__(SORT_NB_HUGE)
 k_tile_colsum(uint32_t tiles, const uint32_t* __restrict__ H, uint32_t* __restrict__ S)
 {
-    const uint32_t t0 = blockIdx.x * SORT_CHUNK, t1 = min(t0 + (uint32_t)SORT_CHUNK, tiles);
+    const uint32_t nb = blockDim.x, t0 = blockIdx.x * SORT_CHUNK, t1 = min(t0 + (uint32_t)SORT_CHUNK, tiles);
     uint32_t sum = 0;
-    for (uint32_t t = t0; t < t1; ++t) sum += H[(size_t)t * SORT_MAX_BUCKETS + threadIdx.x];
-    S[(size_t)blockIdx.x * SORT_MAX_BUCKETS + threadIdx.x] = sum;
+    for (uint32_t t = t0; t < t1; ++t) sum += H[(size_t)t * nb + threadIdx.x];
+    S[(size_t)blockIdx.x * nb + threadIdx.x] = sum;
 }
 
-__global__ void __launch_bounds__(SORT_MAX_BUCKETS)
+__global__ void __launch_bounds__(SORT_NB_HUGE)
 k_tile_chunkscan(uint32_t chunks, uint32_t* __restrict__ S)
 {
+    const uint32_t nb = blockDim.x;
     uint32_t run = 0;
     for (uint32_t ch = 0; ch < chunks; ++ch) {
-        const size_t i = (size_t)ch * SORT_MAX_BUCKETS + threadIdx.x;
+        const size_t i = (size_t)ch * nb + threadIdx.x;
         const uint32_t v = S[i];
         S[i] = run;
         run += v;
     }
 }
 
-__global__ void __launch_bounds__(SORT_MAX_BUCKETS)
+__global__ void __launch_bounds__(SORT_NB_HUGE)
 k_tile_colscan(uint32_t tiles, int shift, const uint32_t* __restrict__ H, const uint32_t* __restrict__ S,
                uint32_t* __restrict__ Hs)
 {
-    const uint32_t t0 = blockIdx.x * SORT_CHUNK, t1 = min(t0 + (uint32_t)SORT_CHUNK, tiles);
-    uint32_t run = (threadIdx.x << shift) + S[(size_t)blockIdx.x * SORT_MAX_BUCKETS + threadIdx.x];
+    const uint32_t nb = blockDim.x, t0 = blockIdx.x * SORT_CHUNK, t1 = min(t0 + (uint32_t)SORT_CHUNK, tiles);
+    uint32_t run = (threadIdx.x << shift) + S[(size_t)blockIdx.x * nb + threadIdx.x];
     for (uint32_t t = t0; t < t1; ++t) {
-        const size_t i = (size_t)t * SORT_MAX_BUCKETS + threadIdx.x;
+        const size_t i = (size_t)t * nb + threadIdx.x;
         const uint32_t v = H[i];
         Hs[i] = run;
         run += v;
@@ -288,32 +297,33 @@ struct Sort7 { const double* in[7]; };
 
 // step A: the records of one tile.  T: where bucket b starts in the tile's bucket order, Hs: the first slot of the tile's
 // share of bucket b.
-__global__ void __launch_bounds__(SORT_STAGE_THREADS, 5)
+template <int NB, int TILE>
+__global__ void __launch_bounds__(NB, NB == SORT_NB_SMALL ? 5 : (NB == SORT_NB_LARGE ? 2 : 1))
 k_stage_records(uint32_t n, const uint32_t* __restrict__ dest, const uint32_t* __restrict__ T,
                 const uint32_t* __restrict__ Hs, int shift, Sort7 a, double* __restrict__ tmp,
                 uint32_t* __restrict__ tmpdest)
 {
     extern __shared__ __align__(16) unsigned char stage_smem[];
     double* rec = reinterpret_cast<double*>(stage_smem);
-    uint32_t* slot = reinterpret_cast<uint32_t*>(rec + (size_t)SORT_TILE * 8);   // slot of the record at tile position lp
-    uint32_t* base = slot + SORT_TILE;          // first slot of this tile's share of bucket b
-    uint32_t* toff = base + SORT_MAX_BUCKETS;   // where bucket b starts in the tile's bucket order
-    uint32_t* cnt = toff + SORT_MAX_BUCKETS;    // arrivals so far
-    static_assert(SORT_MAX_BUCKETS == SORT_STAGE_THREADS, "one thread per bucket");
+    uint32_t* slot = reinterpret_cast<uint32_t*>(rec + (size_t)TILE * 8);   // slot of the record at tile position lp
+    uint32_t* base = slot + TILE;          // first slot of this tile's share of bucket b
+    uint32_t* toff = base + NB;   // where bucket b starts in the tile's bucket order
+    uint32_t* cnt = toff + NB;    // arrivals so far
+    constexpr int PER_THREAD = TILE / NB;
     {
-        const size_t row = (size_t)blockIdx.x * SORT_MAX_BUCKETS + threadIdx.x;
+        const size_t row = (size_t)blockIdx.x * NB + threadIdx.x;
         toff[threadIdx.x] = T[row];
         base[threadIdx.x] = Hs[row];
         cnt[threadIdx.x] = 0u;
     }
-    const size_t p0 = (size_t)blockIdx.x * SORT_TILE;
-    const uint32_t tile_n = (uint32_t)min((size_t)SORT_TILE, (size_t)n - p0);
-    // load phase: all 7 x SORT_PER_THREAD values of this thread are requested before the first is used
-    double v[SORT_PER_THREAD][7];
-    uint32_t d[SORT_PER_THREAD];
+    const size_t p0 = (size_t)blockIdx.x * TILE;
+    const uint32_t tile_n = (uint32_t)min((size_t)TILE, (size_t)n - p0);
+    // load phase: all 7 x PER_THREAD values of this thread are requested before the first is used
+    double v[PER_THREAD][7];
+    uint32_t d[PER_THREAD];
 #pragma unroll
-    for (int j = 0; j < SORT_PER_THREAD; ++j) {
-        const uint32_t e = threadIdx.x + j * SORT_STAGE_THREADS;
+    for (int j = 0; j < PER_THREAD; ++j) {
+        const uint32_t e = threadIdx.x + j * NB;
         if (e < tile_n) {
             d[j] = dest[p0 + e];
 #pragma unroll
@@ -322,8 +332,8 @@ k_stage_records(uint32_t n, const uint32_t* __restrict__ dest, const uint32_t* _
     }
     __syncthreads();
 #pragma unroll
-    for (int j = 0; j < SORT_PER_THREAD; ++j) {
-        const uint32_t e = threadIdx.x + j * SORT_STAGE_THREADS;
+    for (int j = 0; j < PER_THREAD; ++j) {
+        const uint32_t e = threadIdx.x + j * NB;
         if (e < tile_n) {
             const uint32_t bk = d[j] >> shift;
             const uint32_t r = atomicAdd(&cnt[bk], 1u);
@@ -342,12 +352,12 @@ k_stage_records(uint32_t n, const uint32_t* __restrict__ dest, const uint32_t* _
     }
     __syncthreads();
     // store phase: 16-byte pieces, consecutive threads = consecutive pieces of consecutive records of a run
-    for (uint32_t t = threadIdx.x; t < tile_n * 4u; t += SORT_STAGE_THREADS) {
+    for (uint32_t t = threadIdx.x; t < tile_n * 4u; t += NB) {
         const uint32_t r = t >> 2, part = t & 3u;
         const double2 pr = *reinterpret_cast<const double2*>(rec + (size_t)r * 8 + 2u * (part ^ ((r >> 1) & 3u)));
         *reinterpret_cast<double2*>(tmp + (size_t)slot[r] * 8 + 2u * part) = pr;
     }
-    for (uint32_t t = threadIdx.x; t < tile_n; t += SORT_STAGE_THREADS)
+    for (uint32_t t = threadIdx.x; t < tile_n; t += NB)
         tmpdest[slot[t]] = (uint32_t)((unsigned long long)__double_as_longlong(rec[(size_t)t * 8 + 2u * (3u ^ ((t >> 1) & 3u)) + 1u]) >> 32);
 }
 

@@ -14,6 +14,8 @@
 """
 from __future__ import annotations
 
+import types
+
 import numpy as np
 import pytest
 import torch
@@ -147,6 +149,26 @@ def test_config4_full_size_sort_is_bit_exact_and_step_matches_oracle():
     V = cfg.dx * cfg.dy * cfg.dz
     for s in range(nsp):
         assert abs(float(rho[s].sum()) * V - qsum[s]) <= 1e-11 * abs(qsum[s])
+    ctx.close()
+
+
+@pytest.mark.parametrize("n,dims", [(40_000_003, (64, 64, 64)), (134_217_729, (128, 128, 128))], ids=["40M_512_buckets", "134M_1024_buckets"])
+def test_sort_of_larger_species_in_arbitrary_order_is_bit_exact(n, dims):
+    """The two larger geometries of the record-based sort (sort.cuh: 512 buckets x tiles of 1024 above 2^25 particles, 1024
+    buckets x tiles of 2048 above 2^26), which no BASELINE.json config reaches in random order: uniform random particles,
+    a ragged last tile and bucket; same bit-exact checks as configs[4]."""
+    _need(40 if n > 100_000_000 else 16)
+    g = torch.Generator(device="cuda")
+    g.manual_seed(n)
+    cfg = types.SimpleNamespace(nx=dims[0], ny=dims[1], nz=dims[2], dx=1.0, dy=0.5, dz=2.0, cells=dims[0] * dims[1] * dims[2])
+    part = {k: torch.rand(n, dtype=torch.float64, device="cuda", generator=g) for k in PKEYS}
+    part["x"] *= cfg.nx * cfg.dx
+    part["y"] *= cfg.ny * cfg.dy
+    part["z"] *= cfg.nz * cfg.dz
+    ctx = pk.Ecsim(*grid_of(cfg), 1)
+    ctx.set_workspace(n)
+    ctx.load_particles(0, -1.0, part, sorted=False)
+    _check_sort_bit_exact(cfg, ctx, 0, part, f"{n} random particles")
     ctx.close()
 
 
