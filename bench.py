@@ -468,14 +468,18 @@ def measure_sustained(args, cfg, ctx, restore_arrays, work, E, B, rho, J, M, n_s
     """n_steps CONSECUTIVE steps, fields fixed, particle state never restored (configs[1]'s protocol; 10 steps of the
     headline workload by default): every stray, re-sort and fresh layout is inside the timed steps.
       dense:    the caller's arrays pushed in place (ecsim_push_and_moments_all): leavers become strays, re-sorts by rent-or-buy
-      resident: library-managed gapped double buffers (ecsim_make_resident): the sort-preserving push, no strays."""
+      resident: library-managed gapped double buffers (ecsim_make_resident): the sort-preserving push, no strays.
+      resident_split: the same species stepped as a real ECsim time step does: ecsim_moments_all, [the field
+                solve would run here], ecsim_push_all -- two passes over the particles instead of one."""
     import torch
     import paper_2603_16624_b200 as pk
     nsp = len(cfg.species)
     out = {}
-    for kind in ("dense", "resident"):
+    for kind in ("dense", "resident", "resident_split"):
         restore_arrays()
-        if kind == "resident":
+        if kind != "dense":
+            torch.cuda.synchronize()
+            torch.cuda.empty_cache()              # the gapped buffers of the previous kind go back to the driver
             free, _ = torch.cuda.mem_get_info()
             need = sum(ctx.resident_bytes(int(work[s]["x"].numel()), 0.5) for s in range(nsp))
             if need > free - (2 << 30):
@@ -489,7 +493,11 @@ def measure_sustained(args, cfg, ctx, restore_arrays, work, E, B, rho, J, M, n_s
         for _ in range(n_steps):
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record()
-            ctx.push_and_moments_all(E, B, cfg.dt, cfg.theta, rho, J, M, accumulate=pk.ACC_NONE)
+            if kind == "resident_split":
+                ctx.moments_all(B, cfg.dt, rho, J, M, accumulate=pk.ACC_NONE)
+                ctx.push_all(E, B, cfg.dt, cfg.theta)
+            else:
+                ctx.push_and_moments_all(E, B, cfg.dt, cfg.theta, rho, J, M, accumulate=pk.ACC_NONE)
             e1.record()
             torch.cuda.synchronize()
             ms.append(e0.elapsed_time(e1))
