@@ -914,7 +914,7 @@ extern "C" int64_t ecsim_leaver_count(ecsim_ctx* c)
 template <int NW, int REGS, int MODE, int LAYOUT>
 static cudaError_t launch_fused(const ecsim_ctx* c, const FusedArgs& fa)
 {
-    const size_t smem = (size_t)NW * (MODE == MODE_PUSH ? FLD_DOUBLES : WARP_SMEM_DOUBLES) * sizeof(double);
+    const size_t smem = (size_t)NW * fused_warp_doubles(MODE, LAYOUT) * sizeof(double);
     // per launch, not per process: a second device of the same process needs its own opt-in
     cudaError_t e = cudaFuncSetAttribute(k_fused_push_moments<NW, REGS, MODE, LAYOUT>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

@@ -67,6 +67,14 @@ constexpr int AJ_PER_CELL = 32;
 constexpr int AD_PER_CELL = 128; // MODE_DIAG: [8 corners][16]: rho, J[3], P[6] (xx,xy,xz,yy,yz,zz), Q[3], 3 pad
 constexpr int ROW_D = 0;         // MODE_DIAG: rows 0..15 = the 16 columns (1, v, v v^T, |v|^2/2 v, 0, 0, 0) of the two B tiles
 constexpr unsigned CELL_WEIGHT = 8;   // schedule weight of a cell, in particles
+constexpr int LQ_CAP = 64;            // GAPPED push: leavers waiting in a warp's shared-memory queue (flushed 32 at a time)
+constexpr int LQ_DOUBLES = 8 * LQ_CAP;   // [x,y,z,u,v,w,q,species][LQ_CAP]
+// shared memory of one warp of k_fused_push_moments<.., MODE, LAYOUT>, in doubles
+__host__ __device__ constexpr int fused_warp_doubles(int mode, int layout)
+{
+    return (mode == MODE_PUSH ? FLD_DOUBLES : WARP_SMEM_DOUBLES) +
+           ((layout == LAYOUT_GAPPED && (mode == MODE_FUSED || mode == MODE_PUSH)) ? LQ_DOUBLES : 0);
+}
 
 struct SpeciesDev {
     const uint32_t* seg;     // [cells+1]: DENSE start table; GAPPED first slot of every cell's segment
@@ -353,7 +361,8 @@ k_fused_push_moments(const __grid_constant__ FusedArgs a)
     constexpr bool DIAG = MODE == MODE_DIAG;
     constexpr bool DEPOSIT = MODE == MODE_FUSED || MODE == MODE_MOMENTS, PUSH = MODE == MODE_FUSED || MODE == MODE_PUSH;
     constexpr bool GAPPED = LAYOUT == LAYOUT_GAPPED, TILE = DEPOSIT || DIAG;
-    constexpr int WSM = TILE ? WARP_SMEM_DOUBLES : FLD_DOUBLES;
+    constexpr int WSM = fused_warp_doubles(MODE, LAYOUT);
+    constexpr bool QUEUE = GAPPED && PUSH;
 
     double* stg = smem + (size_t)warp * WSM;
     double* fld = TILE ? stg + ST_ROWS * ST_PITCH : stg;
@@ -378,6 +387,29 @@ k_fused_push_moments(const __grid_constant__ FusedArgs a)
     const double* frag = stg + fr * ST_PITCH + fk;
     double* stcol = stg + lane;
     const unsigned lt_mask = (1u << lane) - 1u;
+
+    // GAPPED push: particles that leave their cell wait in a per-warp queue and are placed 32 at a time -- the four table
+    // reads, the arrival ticket and the seven scattered stores of a relocation are two dependent L2 round trips, paid once
+    // per 32 leavers instead of once per batch that holds one (31 % of the batches at 1.2 % leavers, 70 % at 3.7 %)
+    double* lq = stg + (TILE ? WARP_SMEM_DOUBLES : FLD_DOUBLES);
+    uint32_t qn = 0;
+    auto flush_leavers = [&](uint32_t first, uint32_t count) {
+        const bool mine = (uint32_t)lane < count;
+        const uint32_t e = first + (uint32_t)lane;
+        PushedRegs o;
+        double q = 0.0;
+        int sidx = -1;
+        if (mine) {
+            o.x = lq[e]; o.y = lq[LQ_CAP + e]; o.z = lq[2 * LQ_CAP + e];
+            o.u = lq[3 * LQ_CAP + e]; o.v = lq[4 * LQ_CAP + e]; o.w = lq[5 * LQ_CAP + e];
+            q = lq[6 * LQ_CAP + e];
+            sidx = (int)lq[7 * LQ_CAP + e];
+        }
+        o.stays = false;
+        for (int t = 0; t < nsp; ++t)
+            if (mine && sidx == t) relocate(g, a.sp[t], o, q);
+        __syncwarp();
+    };
 
     // field staging: lane t and t+32 (< 48) hold corner t/6, component t%6 of the next cell
     const int fc0 = lane / 6, fk0 = lane - fc0 * 6;
@@ -535,7 +567,20 @@ k_fused_push_moments(const __grid_constant__ FusedArgs a)
                         sp.ou[d] = o.u; sp.ov[d] = o.v; sp.ow[d] = o.w; sp.oq[d] = cur.q;
                     }
                     nstay += (uint32_t)__popc(smask);
-                    if (inside && !o.stays) { relocate(g, sp, o, cur.q); my_leavers += 1u; }
+                    const bool leave = inside && !o.stays;
+                    const unsigned lmask = __ballot_sync(0xffffffffu, leave);
+                    if (lmask) {
+                        if (leave) {
+                            const uint32_t e = qn + (uint32_t)__popc(lmask & lt_mask);
+                            lq[e] = o.x; lq[LQ_CAP + e] = o.y; lq[2 * LQ_CAP + e] = o.z;
+                            lq[3 * LQ_CAP + e] = o.u; lq[4 * LQ_CAP + e] = o.v; lq[5 * LQ_CAP + e] = o.w;
+                            lq[6 * LQ_CAP + e] = cur.q; lq[7 * LQ_CAP + e] = (double)s;
+                            my_leavers += 1u;
+                        }
+                        qn += (uint32_t)__popc(lmask);
+                        __syncwarp();
+                        if (qn >= 32u) { flush_leavers(qn - 32u, 32u); qn -= 32u; }
+                    }
                 } else if (inside) {
                     sp.u[p] = o.u; sp.v[p] = o.v; sp.w[p] = o.w;
                     sp.x[p] = o.x; sp.y[p] = o.y; sp.z[p] = o.z;
@@ -676,5 +721,6 @@ k_fused_push_moments(const __grid_constant__ FusedArgs a)
             }
         }
     }
+    if (QUEUE && qn) flush_leavers(0u, qn);
     if (PUSH && lane < nsp && lv_acc) atomicAdd(a.sp[lane].leavers, lv_acc);
 }
