@@ -76,7 +76,7 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
-    ap.add_argument("--cpu-sample-planes", type=int, default=8, help="x-planes of cells the oracle sample covers")
+    ap.add_argument("--cpu-sample-planes", type=int, default=32, help="x-planes of cells the oracle sample covers")
     ap.add_argument("--no-rows", action="store_true", help="skip the timings of the separate SURVEY 8(f) calls (moments, push, apply_M, diagnostics)")
     ap.add_argument("--sustained-steps", type=int, default=-1,
                     help="consecutive steps WITHOUT restoring the particle state (default: 10; configs[1]: its 1 + 10 protocol; 0 = skip)")
