@@ -13,7 +13,7 @@ restored from a pristine device copy between steps, outside the timed region; th
 (15 GB of particles, 4 GB of M) is far larger than the 126 MB L2, so no explicit flush is needed.
 
 One JSON line on stdout (rank 0).  `--impl reference` times the CPU oracle (oracle/, as it
-stands, single thread) on a bounded sample of the same workload instead.
+stands, all host cores) on a bounded sample of the same workload instead.
 """
 from __future__ import annotations
 
@@ -194,7 +194,8 @@ def oracle_sample(cfg, planes, all_cores=True):
     plane_start[planes:] = plane_start[planes]           # planes beyond the sample hold no particles
     mom = oracle.Moments(cfg.nodes, with_abs=False)      # calloc-backed: only touched pages are committed
     oracle.lib()
-    threads = oracle.threads() if all_cores else 1
+    # planes of one colour run in parallel: at most ceil(planes / 2) threads have work
+    threads = min(oracle.threads(), (planes + 1) // 2) if all_cores else 1
     t0 = time.perf_counter()
     for s, sp in enumerate(cfg.species):
         if all_cores:
