@@ -115,7 +115,7 @@ def sum_over_ranks(value, world, backend_device="cuda"):
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
 
-    QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+    QUERY = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
              "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
@@ -131,7 +131,10 @@ class ClockSampler:
         except Exception:
             self.proc = None
 
-    def stop(self):
+    def stop(self, t_begin=None, t_end=None):
+        """Summary of the samples whose nvidia-smi timestamp lies in [t_begin, t_end] (time.time() values; the sampler is
+        started long before, because nvidia-smi needs a few tenths of a second for its first line)."""
+        import datetime
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         self.proc.terminate()
@@ -146,6 +149,13 @@ class ClockSampler:
             f = [x.strip() for x in line.split(",")]
             if len(f) < 9:
                 continue
+            if t_begin is not None:
+                try:
+                    ts = datetime.datetime.strptime(f[0], "%Y/%m/%d %H:%M:%S.%f").timestamp()
+                except ValueError:
+                    continue
+                if ts < t_begin - 0.03 or ts > t_end + 0.03:
+                    continue
             try:
                 sm.append(float(f[1])); smax.append(float(f[2])); power.append(float(f[3]))
             except ValueError:
@@ -249,6 +259,8 @@ def run_product(args):
         from paper_2603_16624_b200 import build as product_build
         product_build.build()                     # in-tree, only if missing or stale; other ranks wait at the barrier below
     torch.cuda.set_device(local % torch.cuda.device_count())
+    sampler = ClockSampler(local % torch.cuda.device_count())
+    sampler.start()
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl")
@@ -300,15 +312,15 @@ def run_product(args):
 
     fp64_probe, _ = ctx.probe_fp64(4096)
 
+    # clock samples: nvidia-smi needs a few tenths of a second for its first line, so it was started with the process; the
+    # samples kept are those stamped between the first warm-up step (same load as the timed ones) and the last timed step
+    t_clock0 = time.time()
     for _ in range(max(3, args.warmup)):
         restore()
         one_step()
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
-
-    sampler = ClockSampler(torch.cuda.current_device())
-    sampler.start()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     kernel_ms = []
     launches0 = ctx.launch_count()
@@ -327,7 +339,7 @@ def run_product(args):
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
-    clocks = sampler.stop()
+    clocks = sampler.stop(t_clock0, time.time())
     step_ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = max_over_ranks([sum(step_ms)], world)[0]
     ms_per_step = total_ms / args.steps
