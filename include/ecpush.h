@@ -263,6 +263,41 @@ int ecsim_probe_fp64(ecsim_ctx *ctx, int iters, double *tflops_out, float *ms_ou
 
 int ecsim_destroy(ecsim_ctx *ctx);
 
+/* Per-cell segment table of a species WITHOUT a context, a workspace or any allocation: the binning of L131 and the
+ * histogram + exclusive scan that open the counting sort (L149), i.e. what ecsim_sort_particles / ecsim_build_segments
+ * compute into the lent workspace.
+ *
+ * Who this is for.  Everything else in this header needs a context (ecsim_init_grid creates events and pinned host
+ * buffers) and scratch that the caller obtained from cudaMalloc and lent with ecsim_set_workspace.  Some callers cannot do
+ * that: a plug-in called from inside a host code whose device memory is handed out once at start-up (ECsim's own OpenACC
+ * data regions, or a framework whose pool already holds the whole HBM, so that a fresh cudaMalloc fails or evicts);
+ * code on a latency-critical path of a time loop, where cudaMalloc / cudaFree serialise the whole device; code running
+ * under a memory budget fixed by a scheduler.  This call lets them bin a species with nothing but their own input and
+ * output arrays.  Its scratch (the cell histogram and the partial sums of the scan) lives in an array compiled into the
+ * library, ECSIM_STATIC_MAX_CELLS + 4096 32-bit words = 8.02 MB, which every GPU that loads libecpush holds from the
+ * load of the library's device code until the process exits, whether or not this call is ever made.
+ *
+ *   cuda_stream    cudaStream_t (NULL = legacy default stream) of the CURRENT device; all work is enqueued on it
+ *   nx, ny, nz     cells per axis, each >= 2, with nx*ny*nz <= ECSIM_STATIC_MAX_CELLS (128^3, the largest BASELINE.json
+ *                  grid); a larger grid is refused with ECSIM_ERR_INVALID_ARG and a text in ecsim_last_error() that
+ *                  names the limit -- nothing is enqueued
+ *   dx, dy, dz     spacing > 0 (cell of a particle as in the conventions above: floor(x * (1/dx)) per axis, clamped)
+ *   n, x, y, z     n >= 0 particles (n < 2^32), device arrays of n doubles, read only, any order
+ *   cell_count_out device int32[cells]: particles per cell (what ecsim_sort_particles returns); or NULL
+ *   start_out      device uint32[cells+1]: exclusive running sum of the counts, start_out[cells] = n; or NULL
+ *                  (at least one of the two outputs must be given)
+ *
+ * The call makes no cudaMalloc / cudaFree / cudaMallocHost, creates no stream or event and calls no library routine that
+ * allocates; it does not synchronise.  The FIRST call on each device looks up that device's address of the built-in
+ * array (cudaGetSymbolAddress, which may load the library's device code): make that first call outside any stream
+ * capture.  All calls on one device share the one array: the call clears the histogram itself before counting, but two
+ * calls whose work can overlap on the GPU (different streams without an ordering between them, or two host threads
+ * on different streams) race on it and both results are undefined -- order them on one stream or with events. */
+#define ECSIM_STATIC_MAX_CELLS 2097152
+int ecsim_cell_segments_static(void *cuda_stream, int nx, int ny, int nz, double dx, double dy, double dz,
+                               int64_t n, const double *x, const double *y, const double *z,
+                               int32_t *cell_count_out, uint32_t *start_out);
+
 /* Static text for a status; ecsim_last_error: text of the last CUDA failure in this process. */
 const char *ecsim_strerror(int status);
 const char *ecsim_last_error(void);

@@ -20,4 +20,6 @@ from .binding import (  # noqa: F401
     ACC_M_ONLY,
     M_27,
     M_14,
+    STATIC_MAX_CELLS,
+    cell_segments_static,
 )

@@ -22,6 +22,7 @@ ACC_ALL = 1
 ACC_M_ONLY = 2
 M_27 = 0
 M_14 = 1
+STATIC_MAX_CELLS = 2097152      # ECSIM_STATIC_MAX_CELLS of ecpush.h: the grid the built-in scratch can serve
 
 _c = ctypes
 _P = _c.c_void_p
@@ -86,6 +87,8 @@ _PROTOS = {
     "ecsim_resort_count": (_c.c_int64, [_P]),
     "ecsim_probe_fp64": (_c.c_int, [_P, _c.c_int, _c.POINTER(_c.c_double), _c.POINTER(_c.c_float)]),
     "ecsim_destroy": (_c.c_int, [_P]),
+    "ecsim_cell_segments_static": (_c.c_int, [_P, _c.c_int, _c.c_int, _c.c_int, _c.c_double, _c.c_double, _c.c_double,
+                                              _c.c_int64, _P, _P, _P, _P, _P]),
     "ecsim_strerror": (_c.c_char_p, [_c.c_int]),
     "ecsim_last_error": (_c.c_char_p, []),
 }
@@ -133,6 +136,24 @@ def _hptr(t, dtype=None):
     if dtype is not None and t.dtype != dtype:
         raise EcsimError(f"expected dtype {dtype}, got {t.dtype}")
     return _P(t.data_ptr())
+
+
+def cell_segments_static(nx: int, ny: int, nz: int, dx: float, dy: float, dz: float, x, y, z,
+                         cell_count_out=None, start_out=None, stream=None):
+    """ecsim_cell_segments_static: per-cell counts (int32[cells]) and / or the segment table (uint32[cells+1], stored in
+    an int32 or uint32 tensor) of the particles at x, y, z, for callers that cannot allocate device memory: no context,
+    no workspace, the scratch is an array built into libecpush.so (grids up to STATIC_MAX_CELLS cells).  Work is
+    enqueued on `stream` (default: torch's current stream); calls that may overlap on the GPU race on the shared scratch."""
+    import torch
+    f64 = torch.float64
+    n = int(x.numel())
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    if start_out is not None and start_out.dtype not in (torch.int32, torch.uint32):
+        raise EcsimError(f"start_out: expected a 32-bit integer tensor, got {start_out.dtype}")
+    _check(lib().ecsim_cell_segments_static(_P(stream.cuda_stream), nx, ny, nz, dx, dy, dz, n, _dptr(x, f64),
+                                            _dptr(y, f64), _dptr(z, f64), _dptr(cell_count_out, torch.int32),
+                                            _dptr(start_out)), "ecsim_cell_segments_static")
 
 
 class Ecsim:

@@ -7,6 +7,7 @@
 #include <stdlib.h>
 #include <string.h>
 #include <algorithm>
+#include <mutex>
 #include <new>
 
 #include "../../include/ecpush.h"
@@ -1641,5 +1642,129 @@ extern "C" int ecsim_probe_fp64(ecsim_ctx* c, int iters, double* tflops_out, flo
     const double flops = 2.0 * PROBE_CHAINS * PROBE_UNROLL * (double)iters * blocks * threads;
     *tflops_out = flops / (ms * 1e-3) * 1e-12;
     if (ms_out) *ms_out = ms;
+    return ECSIM_OK;
+}
+
+// --------------------------------------------------------------------------------------------
+// ecsim_cell_segments_static (ecpush.h): the histogram + exclusive scan of the counting sort for callers that cannot
+// obtain device memory -- a plug-in inside a host code whose HBM is handed out once at start-up (OpenACC data regions, a
+// framework pool that holds the whole card), or a time loop that must not take the device-wide stall of cudaMalloc /
+// cudaFree.  Nothing is allocated here, on either side of the bus: the scratch that the context-based path carves from
+// the lent workspace (Workspace::count, Workspace::block_sums) is this file-scope array, part of the library's device
+// image, 8.02 MB on every GPU that loads it, until the process exits.
+//
+// g_static_scratch is a DEVICE symbol.  In the host code below the name is only the host-side handle the runtime
+// registers for it; handing `g_static_scratch` itself to a kernel would give the kernel a host address.  The address
+// a kernel can use comes from cudaGetSymbolAddress, taken once per device with that device current (each device has
+// its own copy of the array at its own address), and that is the only pointer passed on.
+constexpr size_t STATIC_SUMS_WORDS = 4096;    // block sums of the scan: ECSIM_STATIC_MAX_CELLS / SCAN_BLOCK + 1 = 2049 used
+constexpr size_t STATIC_SCRATCH_WORDS = (size_t)ECSIM_STATIC_MAX_CELLS + STATIC_SUMS_WORDS;
+static_assert(ECSIM_STATIC_MAX_CELLS / SCAN_BLOCK + 1 <= STATIC_SUMS_WORDS, "block sums of the largest grid must fit");
+static_assert(((size_t)ECSIM_STATIC_MAX_CELLS * sizeof(uint32_t)) % 256 == 0, "block sums start 256-byte aligned");
+static __device__ __align__(256) uint32_t g_static_scratch[STATIC_SCRATCH_WORDS];
+
+constexpr int STATIC_MAX_DEVICES = 64;
+struct StaticScratchOfDevice {
+    uint32_t* dev_ptr = nullptr;   // device address of this device's copy of g_static_scratch
+    int sm_count = 0;
+};
+static StaticScratchOfDevice g_static_of_device[STATIC_MAX_DEVICES];
+static std::mutex g_static_mutex;
+
+// Set-up, once per device, with that device current: the device address of the array and the SM count (grid sizing).
+// cudaGetSymbolAddress allocates nothing (the array came with the device image); it may load that image, which is why
+// the first call on a device belongs outside a stream capture.
+static int static_scratch_of_current_device(uint32_t** ptr_out, int* sm_count_out)
+{
+    int dev = -1;
+    CK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) {
+        snprintf(g_last_error, sizeof(g_last_error),
+                 "ecsim_cell_segments_static: device ordinal %d outside the %d devices this build keeps an address for",
+                 dev, STATIC_MAX_DEVICES);
+        return ECSIM_ERR_INVALID_ARG;
+    }
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticScratchOfDevice& d = g_static_of_device[dev];
+    if (!d.dev_ptr) {
+        int sms = 0;
+        CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        uint32_t* p = nullptr;
+        CK(cudaGetSymbolAddress(reinterpret_cast<void**>(&p), g_static_scratch));
+        if (!p || sms < 1) {
+            snprintf(g_last_error, sizeof(g_last_error),
+                     "ecsim_cell_segments_static: no device address for the built-in scratch on device %d", dev);
+            return ECSIM_ERR_CUDA;
+        }
+        d.sm_count = sms;
+        d.dev_ptr = p;             // last: a non-null pointer marks the device as set up
+    }
+    *ptr_out = d.dev_ptr;
+    *sm_count_out = d.sm_count;
+    return ECSIM_OK;
+}
+
+extern "C" int ecsim_cell_segments_static(void* cuda_stream, int nx, int ny, int nz, double dx, double dy, double dz,
+                                          int64_t n, const double* x, const double* y, const double* z,
+                                          int32_t* cell_count_out, uint32_t* start_out)
+{
+    if (nx < 2 || ny < 2 || nz < 2 || !(dx > 0) || !(dy > 0) || !(dz > 0) || n < 0 || n >= 0xffffffffLL)
+        return ECSIM_ERR_INVALID_ARG;
+    if (n > 0 && (!x || !y || !z)) return ECSIM_ERR_INVALID_ARG;
+    if (!cell_count_out && !start_out) return ECSIM_ERR_INVALID_ARG;
+    const long long cells_ll = (long long)nx * ny * nz;
+    if (cells_ll > (long long)ECSIM_STATIC_MAX_CELLS) {
+        // refused before anything is enqueued: the built-in scratch cannot grow
+        snprintf(g_last_error, sizeof(g_last_error),
+                 "ecsim_cell_segments_static: grid %d x %d x %d = %lld cells exceeds the built-in scratch of "
+                 "ECSIM_STATIC_MAX_CELLS = %d cells; use a context with a lent workspace (ecsim_sort_particles) for "
+                 "larger grids", nx, ny, nz, cells_ll, (int)ECSIM_STATIC_MAX_CELLS);
+        return ECSIM_ERR_INVALID_ARG;
+    }
+    uint32_t* scratch = nullptr;
+    int sm_count = 0;
+    int rc = static_scratch_of_current_device(&scratch, &sm_count);
+    if (rc) return rc;
+
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+    const uint32_t cells = (uint32_t)cells_ll;
+    uint32_t* count = scratch;                                  // [cells]   histogram
+    uint32_t* block_sums = scratch + ECSIM_STATIC_MAX_CELLS;    // [nb + 1]  partial sums of the scan
+    Geom g;                                                     // as ecsim_init_grid forms it: same binning, bit for bit
+    g.nx = nx; g.ny = ny; g.nz = nz;
+    g.dx = dx; g.dy = dy; g.dz = dz;
+    g.rdx = 1.0 / dx; g.rdy = 1.0 / dy; g.rdz = 1.0 / dz;
+    g.Lx = nx * dx; g.Ly = ny * dy; g.Lz = nz * dz;
+    g.invV = 1.0 / (dx * dy * dz);
+    g.nodes = cells_ll;
+    g.fix_mask = 0;
+    g.fix_pos[0] = g.fix_pos[1] = g.fix_pos[2] = 0.0;
+
+    // The array keeps whatever the previous call left in it: the histogram is accumulated with atomics and must start at
+    // zero; the block sums are overwritten by k_scan_blocks before they are read and need no clearing.
+    CK(cudaMemsetAsync(count, 0, sizeof(uint32_t) * cells, st));
+    if (n > 0) {
+        size_t blocks = ((size_t)n + 255) / 256;
+        const size_t cap = (size_t)sm_count * 16;
+        if (blocks > cap) blocks = cap;
+        k_cell_hist<false><<<(int)blocks, 256, 0, st>>>(g, (uint32_t)n, x, y, z, nullptr, nullptr, count);
+        CK_LAUNCH();
+    }
+    if (cell_count_out) {
+        size_t blocks = ((size_t)cells + 255) / 256;
+        const size_t cap = (size_t)sm_count * 16;
+        if (blocks > cap) blocks = cap;
+        k_copy_u32_to_i32<<<(int)blocks, 256, 0, st>>>(cells, count, cell_count_out);
+        CK_LAUNCH();
+    }
+    if (start_out) {
+        const uint32_t nb = (cells + SCAN_BLOCK - 1) / SCAN_BLOCK;
+        k_scan_blocks<<<nb, SCAN_BLOCK, 0, st>>>(count, start_out, block_sums, cells);
+        CK_LAUNCH();
+        k_scan_sums<<<1, SCAN_BLOCK, 0, st>>>(block_sums, nb, start_out, cells);
+        CK_LAUNCH();
+        k_scan_add<<<nb, SCAN_BLOCK, 0, st>>>(start_out, block_sums, cells);
+        CK_LAUNCH();
+    }
     return ECSIM_OK;
 }
