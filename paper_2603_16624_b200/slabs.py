@@ -12,7 +12,7 @@ How the periodic single-GPU library serves a non-periodic slab: the rank's local
 cells 0..nxl-1 are the slab, plane nxl is the RIGHT ghost and plane nxl+1 the LEFT ghost (it is "plane -1" of the
 periodic local grid).  Particles live only in the slab's cells, so their deposits reach node planes 0..nxl and nothing
 wraps; a particle that leaves to the right ends in ghost plane nxl, one that leaves to the left wraps into ghost plane
-nxl+1 (|displacement| < one cell per step is required and checked).  Local fields carry node planes 0..nxl of the slab
+nxl+1 (a particle must END in the slab or in the plane next to it; leavers() checks that by the sign of the velocity).  Local fields carry node planes 0..nxl of the slab
 (plane nxl = the right neighbour's plane 0: a halo COPY the caller provides from its field solve; local_fields() cuts it
 out of a global array).
 
@@ -77,13 +77,32 @@ class SlabGrid:
         out["x"] = torch.where(x >= L, x - L, x)
         return out
 
-    def leavers(self, part: Dict[str, torch.Tensor]):
+    def leavers(self, part: Dict[str, torch.Tensor], dt: float = None):
         """After a push on the local (periodic, nxl+2 planes) grid: masks of the particles now in the right / left ghost
-        plane, and the same particles packed in the RECEIVER's local coordinates.  [7][n] tensors."""
-        x = part["x"]
+        plane, and the same particles packed in the RECEIVER's local coordinates.  [7][n] tensors.
+
+        A particle may cross several cells in a step (ECsim steps beyond the CFL limit) as long as it ENDS in the slab
+        or in the plane next to it.  One that ends farther out is indistinguishable by position from another particle
+        (from plane nxl-1 by +2 planes it lands in plane nxl+1, the LEFT ghost) and would be handed to the wrong
+        neighbour; it is refused here instead:
+          * always: the sign of the post-push velocity (x_new - x_old = dt u, Eq. 8) must agree with the side of the
+            ghost plane -- this catches an end up to two planes outside the slab;
+          * with `dt` given, exactly: the position the particle came from, x_new - dt u taken in the frame its class
+            implies (left leavers: one period of the local grid lower), must lie in the slab."""
+        x, u = part["x"], part["u"]
         ci = torch.floor(x / self.dx)
         right = ci == self.nxl
         left = ci >= self.nxl + 1
+        refuse = "the slab migration exchanges with the nearest neighbours only (split the step or widen the ghost layer)"
+        if bool((right & (u < 0)).any()) or bool((left & (u > 0)).any()):
+            raise RuntimeError("a particle ended two cell planes outside its slab (its velocity points away from the "
+                               "ghost plane it was found in): " + refuse)
+        if dt is not None and x.numel():
+            origin = x - dt * u - left.to(x.dtype) * ((self.nxl + 2) * self.dx)
+            tol = 1e-9 * self.dx
+            if bool(((origin < -tol) | (origin > self.nxl * self.dx + tol)).any()):
+                raise RuntimeError("a particle ended more than one cell plane outside its slab (x_new - dt u is not "
+                                   "inside the slab): " + refuse)
         stay = ~(right | left)
         pack_r = torch.stack([part[k][right] for k in PKEYS])
         pack_l = torch.stack([part[k][left] for k in PKEYS])

@@ -52,7 +52,7 @@ def test_slab_decomposed_steps_match_single_domain_oracle(world, m_layout):
         for r in range(world):
             grids[r].add_halo(got[r], *out[r])
         for s in range(nsp):
-            packs = [grids[r].leavers(parts[r][s]) for r in range(world)]
+            packs = [grids[r].leavers(parts[r][s], cfg.dt) for r in range(world)]
             fl, fr = ring.exchange([p[1] for p in packs], [p[2] for p in packs])
             moved += sum(int(p[1].shape[1] + p[2].shape[1]) for p in packs)
             for r in range(world):

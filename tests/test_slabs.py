@@ -39,7 +39,7 @@ def run_local_ring(cfg, world, steps, engine):
         for r in range(world):
             grids[r].add_halo(got[r], *out[r])
         for s in range(nsp):
-            packs = [grids[r].leavers(parts[r][s]) for r in range(world)]
+            packs = [grids[r].leavers(parts[r][s], cfg.dt) for r in range(world)]
             fl, fr = ring.exchange([p[1] for p in packs], [p[2] for p in packs])
             moved += sum(int(p[1].shape[1] + p[2].shape[1]) for p in packs)
             for r in range(world):
@@ -77,6 +77,45 @@ def test_slab_grid_bookkeeping():
         SlabGrid(2, 3, 3, 1.0, 1.0, 1.0, 3, 0)
 
 
+def test_a_particle_that_ends_two_planes_out_is_refused_not_misrouted():
+    """ECsim steps beyond the CFL limit, so a particle can cross more than one cell plane in a step.  Ending ONE plane
+    outside the slab after several cells is fine; ending two planes out would look like a leaver to the other side."""
+    g = SlabGrid(12, 2, 2, 0.5, 1.0, 1.0, 3, 1)                 # nxl = 4: slab planes 0..3, right ghost 4, left ghost 5
+    dt = 0.25
+
+    def one(x_old, u):
+        x_new = (x_old + dt * u) % ((g.nxl + 2) * g.dx)         # the push on the periodic local grid
+        p = {k: torch.zeros(1, dtype=torch.float64) for k in PKEYS}
+        p["x"][0], p["u"][0] = x_new, u
+        return p
+
+    # three cells to the right, ending in the right ghost plane: a legitimate right leaver, in the receiver's frame
+    stay, pr, pl = g.leavers(one(0.6, 6.4), dt)                 # 0.6 -> 2.2 = plane 4
+    assert not bool(stay[0]) and pr.shape[1] == 1 and pl.shape[1] == 0 and abs(float(pr[0, 0]) - 0.2) < 1e-12
+    stay, pr, pl = g.leavers(one(0.1, -1.2), dt)                # 0.1 -> -0.2 = plane 5 (left ghost)
+    assert pl.shape[1] == 1 and abs(float(pl[0, 0]) - (g.nxl_left * g.dx - 0.2)) < 1e-12
+    # from the last plane by +2 planes: lands in the LEFT ghost plane with u > 0
+    with pytest.raises(RuntimeError, match="nearest neighbours"):
+        g.leavers(one(1.9, 3.0), dt)                            # 1.9 -> 2.65 = plane 5
+    with pytest.raises(RuntimeError, match="nearest neighbours"):
+        g.leavers(one(1.9, 3.0))                                # the sign check needs no dt
+    # from the first plane by -2 planes: lands in the RIGHT ghost plane with u < 0
+    with pytest.raises(RuntimeError, match="nearest neighbours"):
+        g.leavers(one(0.1, -2.8))                               # 0.1 -> -0.6 = plane 4
+    # a whole period of the local grid and more: the position and the sign look innocent, the origin does not
+    with pytest.raises(RuntimeError, match="nearest neighbours"):
+        g.leavers(one(0.2, 13.0), dt)                           # 0.2 -> 3.45 -> wraps to 0.45: "stayed"
+    # a thermal species with vth dt / dx > 1: some particle always ends too far out
+    rng = torch.Generator().manual_seed(3)
+    n = 4000
+    p = {k: torch.zeros(n, dtype=torch.float64) for k in PKEYS}
+    x_old = torch.rand(n, generator=rng, dtype=torch.float64) * g.nxl * g.dx
+    p["u"] = torch.randn(n, generator=rng, dtype=torch.float64) * (1.5 * g.dx / dt)
+    p["x"] = (x_old + dt * p["u"]) % ((g.nxl + 2) * g.dx)
+    with pytest.raises(RuntimeError, match="nearest neighbours"):
+        g.leavers(p, dt)
+
+
 WORKER = r'''
 import os, sys
 root = os.environ["ECPUSH_ROOT"]
@@ -105,7 +144,7 @@ for step in range(3):
     rho, J, M = oracle_engine(grid, cfg, parts, El, Bl)
     grid.add_halo(ring.shift_right(grid.halo_planes(rho, J, M)), rho, J, M)
     for s in range(nsp):
-        stay, pr, pl = grid.leavers(parts[s])
+        stay, pr, pl = grid.leavers(parts[s], cfg.dt)
         fl, fr = ring.exchange(pr, pl)
         parts[s] = grid.merge(parts[s], stay, fl, fr)
     mine = (grid.owned(rho, 1).clone(), grid.owned(J, 2).clone(), grid.owned(M, 0).clone(),
