@@ -219,7 +219,8 @@ int ecsim_apply_M(ecsim_ctx *ctx, const double *M, const double *E, double *out,
  * call returns ECSIM_ERR_INVALID_ARG (text in ecsim_last_error) and the particle arrays are left partially advanced.
  * Pass sorted = 0 when unsure (serial path, the library sorts).  ecsim_set_host_pipeline(0) forces the serial path, (2)
  * pipelines even tiny inputs (default 1: only when a slab carries >= 32 MB); ecsim_host_pipelined_count = calls that
- * completed through the pipeline. */
+ * completed through the pipeline.  While ecsim_set_fixed_axes is active the serial path is always taken (the particles
+ * are pinned after their upload).  On any error return no copy of the call is still in flight. */
 int ecsim_set_host_pipeline(ecsim_ctx *ctx, int on);
 int64_t ecsim_host_pipelined_count(const ecsim_ctx *ctx);
 size_t ecsim_host_step_workspace_bytes(const ecsim_ctx *ctx, int64_t n_particles);

@@ -383,6 +383,14 @@ extern "C" int ecsim_set_fixed_axes(ecsim_ctx* c, int axis_mask, double px, doub
                 CK_LAUNCH();
                 c->launches++;
             }
+            // ... and the particles without a slot (the overflow list the next pass reads; unused entries do not matter)
+            if (sp.res.ovf_cap > 0) {
+                double* l = sp.res.ovf[sp.res.ovf_cur];
+                const size_t cap = sp.res.ovf_cap;
+                k_fix_position<<<grid_for(c, cap, 256, 16), 256, 0, c->stream>>>(c->g, cap, l, l + cap, l + 2 * cap);
+                CK_LAUNCH();
+                c->launches++;
+            }
             // the pinned particles may now sit in other cells than their segments say: bin and lay out afresh
             rc = resident_relayout(c, s, false);
             if (rc) return rc;
@@ -1524,6 +1532,12 @@ static int host_step_impl(ecsim_ctx* c, int nsp, const int64_t* n, const double*
     tail += align_up(sizeof(double) * 4 * nodes * nsp, 256);
     double* dM = reinterpret_cast<double*>(tail);
     cudaStream_t st = c->stream;
+    // a resident species parked in one of the slots: settle its last push first (restore() below forgets the pending
+    // counters, and with them an ECSIM_ERR_OVERFLOW that has not been reported yet)
+    for (int s = 0; s < nsp; ++s) {
+        const int src = resident_settle(c, s);
+        if (src) return src;
+    }
     SpeciesHost saved[ECSIM_MAX_SPECIES];
     for (int s = 0; s < nsp; ++s) saved[s] = c->sp[s];
 
@@ -1543,7 +1557,10 @@ static int host_step_impl(ecsim_ctx* c, int nsp, const int64_t* n, const double*
             if (c->sp[s].state == ST_SEGMENTED && !c->sp[s].res.on) c->sp[s].state = ST_DECLARED;   // the tables lived in the re-carved buffer
     };
     auto body = [&]() -> int {
-        if (c->host_pipeline && sorted && accumulate == ECSIM_ACC_NONE && c->variant == ECSIM_VARIANT_FUSED) {
+        // (with ecsim_set_fixed_axes active the serial path is taken: its load pins the particles AFTER the upload; the
+        // pipeline's load would pin the still empty staging area while slab 0 is on its way)
+        if (c->host_pipeline && sorted && accumulate == ECSIM_ACC_NONE && c->variant == ECSIM_VARIANT_FUSED &&
+            c->g.fix_mask == 0) {
             double* hp[ECSIM_MAX_SPECIES * 7];
             for (int s = 0; s < nsp; ++s) {
                 double* a7[7] = {hx[s], hy[s], hz[s], hu[s], hv[s], hw[s], const_cast<double*>(hq[s])};
@@ -1593,7 +1610,13 @@ static int host_step_impl(ecsim_ctx* c, int nsp, const int64_t* n, const double*
         return ECSIM_OK;
     };
     const int rc = body();
-    if (rc != ECSIM_OK) cudaStreamSynchronize(st);      // nothing of the failed call may still use the staging area
+    if (rc != ECSIM_OK) {
+        // nothing of the failed call may still use the staging area or the caller's host arrays: the pipeline's
+        // uploads and downloads run on streams of their own
+        cudaStreamSynchronize(st);
+        cudaStreamSynchronize(c->s_up);
+        cudaStreamSynchronize(c->s_down);
+    }
     restore();
     return rc;
 }

@@ -108,3 +108,69 @@ def test_fixed_axes_set_after_the_load_and_switched_off():
     torch.cuda.synchronize()
     assert not bool((pc["z"] == 2.0).all())
     ctx.close()
+
+
+def test_host_step_with_fixed_axes_pins_what_it_uploads():
+    """The host-buffer entry while axes are pinned: the particles arrive unpinned in HOST memory, so the pinning has to
+    happen after the upload.  The pipelined form (which loads before it uploads) must not be taken; forced on, the call
+    still goes through the serial path and equals oracle.fix_position + oracle.step + oracle.fix_position."""
+    cfg = wl.config(0, (8, 6, 4))
+    E, B = wl.gen_fields(cfg)
+    part = wl.gen_species(cfg, 0, shuffle=False)                 # cell-sorted, z anywhere in the box
+    pn = to_numpy(part)
+    host = {k: part[k].clone().pin_memory() for k in PKEYS}
+    ctx = pk.Ecsim(*grid_of(cfg), 1)
+    ctx.set_workspace(part["n"], host_step=True)
+    ctx.set_host_pipeline(2)                                     # "pipeline whatever the size"
+    pz = 2.0 * cfg.dz
+    ctx.set_fixed_axes(4, 0.0, 0.0, pz)
+    rho = torch.full((cfg.nodes,), float("nan"), dtype=torch.float64).pin_memory()
+    J = torch.full((3, cfg.nodes), float("nan"), dtype=torch.float64).pin_memory()
+    M = torch.full((cfg.nodes, 27, 3, 3), float("nan"), dtype=torch.float64).pin_memory()
+    ctx.push_and_moments_host(cfg.species[0].qom, True, host, E.contiguous(), B.contiguous(), cfg.dt, cfg.theta, rho, J, M)
+    assert ctx.host_pipelined_count() == 0
+    oracle.fix_position(pn, 4, 0.0, 0.0, pz)
+    m = oracle.Moments(cfg.nodes)
+    oracle.step(grid_of(cfg), cfg.species[0].qom, cfg.dt, pn, E.numpy(), B.numpy(), m)
+    oracle.fix_position(pn, 4, 0.0, 0.0, pz)
+    assert_moments_close(rho, J, M, m, "host step, z pinned")
+    assert bool((host["z"] == pz).all())
+    assert_particles_close(host, pn, cfg, "host step, z pinned")
+    M7 = M.view(cfg.nx, cfg.ny, cfg.nz, 27, 9)
+    assert float(M7[:, :, [0, 1, 3]].abs().max()) == 0.0         # nothing deposited off the node plane k = 2
+    ctx.close()
+
+
+def test_fixed_axes_on_a_resident_species_pin_its_homeless_particles_too():
+    """A resident species with full segments keeps some particles in its overflow list.  ecsim_set_fixed_axes must pin
+    those as well: the layout that follows puts them back into segments, and anything it missed would stay off the
+    plane until its next push."""
+    base = wl.config(0, (6, 6, 6))
+    hot = tuple(dataclasses.replace(sp, vth=v) for sp, v in zip(base.species, (1.0, 0.5)))
+    cfg = dataclasses.replace(base, dt=0.2, ppc=40, species=hot)
+    E, B = wl.gen_fields(cfg)
+    E_c, B_c = E.cuda(), B.cuda()
+    p = to_numpy(wl.gen_species(cfg, 0))
+    n = p["x"].shape[0]
+    q0 = cfg.species[0].q_sign * cfg.q_abs
+    p["q"] = q0 * (1.0 + np.arange(n) * 2.0 ** -30)
+    ctx = make_ctx(cfg, n, n_species=1)
+    ctx.set_resort_fraction(100.0)                               # never lay out afresh: homeless particles stay homeless
+    ctx.load_particles(0, cfg.species[0].qom, to_cuda(from_numpy(p)), sorted=False)
+    ctx.make_resident(0, 0.0)                                    # no slack: arrivals find their cell full
+    for _ in range(3):
+        ctx.push(0, E_c, B_c, cfg.dt, cfg.theta)
+    assert ctx.relayout_count() == 0
+    pz = 3.0 * cfg.dz
+    ctx.set_fixed_axes(4, 0.0, 0.0, pz)
+    out = {k: torch.empty(n, dtype=torch.float64, device="cuda") for k in PKEYS}
+    ctx.export_particles(0, out)
+    torch.cuda.synchronize()
+    assert np.array_equal(np.sort(_ids(out["q"].cpu().numpy(), q0)), np.arange(n))      # nobody lost
+    assert bool((out["z"] == pz).all()), f"{int((out['z'] != pz).sum())} particle(s) left off the plane"
+    rho = torch.full((cfg.nodes,), float("nan"), dtype=torch.float64, device="cuda")
+    ctx.diagnostics(0, rho, None, None, None)
+    torch.cuda.synchronize()
+    r = rho.view(cfg.nx, cfg.ny, cfg.nz)
+    assert float(r[:, :, [0, 1, 2, 4, 5]].abs().max()) == 0.0
+    ctx.close()
