@@ -26,9 +26,8 @@ import sys
 import time
 
 ROOT = os.path.dirname(os.path.abspath(__file__))
-for _p in (ROOT, os.path.join(ROOT, "tests")):
-    if _p not in sys.path:
-        sys.path.insert(0, _p)
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
 
 METRIC = "particles pushed+mass-matrix-deposited per sec (FP64); % of B200 roofline"
 UNIT = "particles/s"
@@ -192,7 +191,7 @@ def oracle_sample(cfg, planes, all_cores=True):
     import numpy as np
     import oracle
     import workloads as wl
-    from util import grid_of, to_numpy
+    from workloads import grid_of, to_numpy
     planes = max(1, min(planes, cfg.nx))
     cells = list(range(planes * cfg.ny * cfg.nz))
     E, B = wl.gen_fields(cfg)
@@ -250,7 +249,7 @@ def run_product(args):
     import torch
     import paper_2603_16624_b200 as pk
     import workloads as wl
-    from util import PKEYS, grid_of
+    from workloads import PKEYS, grid_of
 
     rank, world, local = dist_env()
     if not torch.cuda.is_available():
@@ -531,7 +530,7 @@ def run_e2e(args, cfg, ctx_unused, pristine, E, B, world):
     host<->device copies inside the timed region."""
     import torch
     import paper_2603_16624_b200 as pk
-    from util import PKEYS, grid_of
+    from workloads import PKEYS, grid_of
     nsp = len(cfg.species)
     n_s = [int(p["x"].numel()) for p in pristine]
     host = [{k: torch.empty(n_s[s], dtype=torch.float64).pin_memory() for k in PKEYS} for s in range(nsp)]

@@ -1,6 +1,6 @@
 // fused_mma.cuh -- the gather / push / deposit kernel for cell-ordered particles.
 //
-// One kernel template, three MODEs and two particle LAYOUTs:
+// One kernel template, four MODEs and two particle LAYOUTs:
 //   MODE_FUSED    deposit (rho, Jhat, M at the pre-push x, v) and push in one pass: E^{n+theta} is an input (north-star)
 //   MODE_MOMENTS  deposit only: x, v untouched (the "moment gathering" block of a real ECsim step)
 //   MODE_PUSH     push only, Eq. 6-8 with the E^{n+theta} the field solve returned (L86-L96)

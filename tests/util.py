@@ -5,16 +5,7 @@ import numpy as np
 
 import workloads as wl
 
-PKEYS = ("x", "y", "z", "u", "v", "w", "q")
-
-
-def grid_of(cfg):
-    return (cfg.nx, cfg.ny, cfg.nz, cfg.dx, cfg.dy, cfg.dz)
-
-
-def to_numpy(part: dict) -> dict:
-    """float64 numpy copies of a generated species (torch tensors, any device)."""
-    return {k: np.ascontiguousarray(part[k].detach().cpu().numpy()).copy() for k in PKEYS}
+from workloads import PKEYS, grid_of, to_numpy  # noqa: F401  (they live in workloads/arrays.py; bench.py uses them too)
 
 
 def rand_particles(rng, n, grid, vscale=1.0, qscale=1.0):

@@ -14,3 +14,4 @@ from .generator import (  # noqa: F401
     cell_layout,
     N_CONFIGS,
 )
+from .arrays import PKEYS, grid_of, to_numpy  # noqa: F401
