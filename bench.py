@@ -77,6 +77,8 @@ def parse_args():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--cpu-sample-planes", type=int, default=32, help="x-planes of cells the oracle sample covers")
     ap.add_argument("--no-rows", action="store_true", help="skip the timings of the separate SURVEY 8(f) calls (moments, push, apply_M, diagnostics)")
+    ap.add_argument("--no-configs", action="store_true",
+                    help="skip the block that times the other BASELINE.json configs (0, 1, 3, 4) and configs[2] with 14 M slots")
     ap.add_argument("--sustained-steps", type=int, default=-1,
                     help="consecutive steps WITHOUT restoring the particle state (default: 10; configs[1]: its 1 + 10 protocol; 0 = skip)")
     return ap.parse_args()
@@ -379,6 +381,14 @@ def run_product(args):
     # ---- what a time loop sees: the step WITH the segment-table build, and consecutive steps ----
     line["step_with_segments_ms"] = measure_with_segments(args, cfg, ctx, restore_arrays, one_step, world)
     line["rows"] = None if args.no_rows else measure_rows(args, cfg, ctx, restore, E, B, rho, J, M, world)
+    headline_run = cfg.idx == 2 and not args.scale and args.variant == "fused" and args.m_layout == 27
+    configs_block = {}
+    if headline_run and not args.no_configs and world == 1:
+        # configs[2] with the paper's 14-slot storage (L73): same particles, same kernel, half the M bytes
+        ctx.set_m_layout(pk.M_14)
+        ms14 = timed_steps(restore, one_step, 3, 5)
+        ctx.set_m_layout(pk.M_27)
+        configs_block["configs[2] m_slots=14"] = config_entry(cfg, n_total, ms14, 14)
     n_sus = args.sustained_steps if args.sustained_steps >= 0 else (cfg.steps if cfg.steps > 1 else 10)
     if n_sus > 0:
         line["sustained"] = measure_sustained(args, cfg, ctx, restore_arrays, work, E, B, rho, J, M, n_sus, n_total, world)
@@ -395,6 +405,13 @@ def run_product(args):
         line["e2e"] = None
     del pristine
     torch.cuda.empty_cache()
+
+    if headline_run and not args.no_configs and world == 1:
+        for idx in (0, 1, 3, 4):
+            configs_block.update(measure_config(idx))
+        line["configs"] = configs_block
+    else:
+        line["configs"] = None
 
     if rank == 0 and not args.no_cpu_baseline and world == 1:
         v, n, dt, cores = oracle_sample(cfg, args.cpu_sample_planes)
@@ -414,6 +431,131 @@ def run_product(args):
 
 def _median(v):
     return statistics.median(v) if v else None
+
+
+def timed_steps(prepare, step, warmup, steps):
+    """Median over `steps` of one call of step(), CUDA events on torch's current stream (the context's stream);
+    prepare() restores the particle state before every step, outside the timed region."""
+    import torch
+    ms = []
+    for i in range(warmup + steps):
+        prepare()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); step(); e1.record()
+        torch.cuda.synchronize()
+        if i >= warmup:
+            ms.append(e0.elapsed_time(e1))
+    return _median(ms)
+
+
+def config_roofline_pps(cfg, n_total, m_slots, with_sort=False):
+    """SURVEY 8(d) applied to a configuration: the slower of the FP64 bound (813 flop per particle) and the HBM bound
+    (104 B per particle + (48 + 32 + 72 m_slots) B per node, at the contract's 8 TB/s); a step that has to sort first
+    adds 144 B per particle of HBM-bound integer work (config 4: 144 B / 8 TB/s + 21.8 ps = 39.8 ps -> 25.1 G/s)."""
+    bytes_pp = 104.0 + (48.0 + 32.0 + 72.0 * m_slots) * cfg.nodes / n_total
+    t = max(bytes_pp / 8.0e12, FLOP_PER_PARTICLE / (FP64_PEAK_TFLOPS * 1e12))
+    if with_sort:
+        t += 144.0 / 8.0e12
+    return 1.0 / t
+
+
+def config_entry(cfg, n_total, ms, m_slots, with_sort=False, **extra):
+    pps = n_total / (ms * 1e-3)
+    roof = config_roofline_pps(cfg, n_total, m_slots, with_sort)
+    out = {"workload": workload_name(cfg), "particles": n_total, "m_slots": m_slots, "ms_per_step": ms,
+           "particles_per_s": pps, "roofline_particles_per_s": roof, "frac": pps / roof,
+           "fits_l2": bool(n_total * 56 < 126e6)}
+    out.update(extra)
+    return out
+
+
+def measure_config(idx):
+    """One of the other BASELINE.json configurations on this GPU, timed like the headline (3 warm-ups, median of 5 steps,
+    particle state restored from a pristine device copy outside the timed region, segment tables built outside):
+      configs[0], [3]  one fused all-species step from the cell-sorted state
+      configs[1]       the same, and its protocol of 1 + 10 consecutive steps with fixed fields, dense and resident
+      configs[4]       particles in random order: the counting sort of both species and the step from the sorted state are
+                       timed separately and summed; `one_call_ms` is ecsim_push_and_moments_all on the
+                       unsorted species (it sorts first), one timed region
+    Configs 0 and 1 fit (partly) in the 126 MB L2: reported, not headline numbers."""
+    import torch
+    import paper_2603_16624_b200 as pk
+    import workloads as wl
+    from workloads import PKEYS, grid_of
+    cfg = wl.config(idx)
+    dev = torch.device("cuda")
+    nsp = len(cfg.species)
+    E, B = wl.gen_fields(cfg, device=dev)
+    pristine = [{k: v.contiguous() for k, v in wl.gen_species(cfg, s, device=dev).items() if k in PKEYS} for s in range(nsp)]
+    n_s = [int(p["x"].numel()) for p in pristine]
+    n_total = sum(n_s)
+    work = [{k: p[k].clone() for k in PKEYS} for p in pristine]
+    ctx = pk.Ecsim(*grid_of(cfg), nsp)
+    ctx.set_workspace(max(n_s))
+    rho = torch.empty(nsp, cfg.nodes, dtype=torch.float64, device=dev)
+    J = torch.empty(nsp, 3, cfg.nodes, dtype=torch.float64, device=dev)
+    M = torch.empty(cfg.nodes, 27, 3, 3, dtype=torch.float64, device=dev)
+
+    def reload(sorted_flag):
+        for s in range(nsp):
+            for k in PKEYS:
+                work[s][k].copy_(pristine[s][k])
+            ctx.load_particles(s, cfg.species[s].qom, work[s], sorted=sorted_flag)
+
+    def restore_sorted():
+        reload(not cfg.shuffled)
+        for s in range(nsp):
+            if cfg.shuffled:
+                ctx.sort_particles(s)
+            else:
+                ctx.build_segments(s)
+
+    def step():
+        ctx.push_and_moments_all(E, B, cfg.dt, cfg.theta, rho, J, M, accumulate=pk.ACC_NONE)
+
+    def sort_all():
+        for s in range(nsp):
+            ctx.sort_particles(s)
+
+    name = f"configs[{idx}]"
+    out = {}
+    if cfg.shuffled:
+        sort_ms = timed_steps(lambda: reload(False), sort_all, 3, 5)
+        push_ms = timed_steps(restore_sorted, step, 3, 5)
+        one_call_ms = timed_steps(lambda: reload(False), step, 2, 5)
+        out[name] = config_entry(cfg, n_total, sort_ms + push_ms, 27, with_sort=True, sort_ms=sort_ms, push_ms=push_ms,
+                                 one_call_ms=one_call_ms, sort_ms_per_species=sort_ms / nsp)
+    else:
+        ms = timed_steps(restore_sorted, step, 3, 5)
+        out[name] = config_entry(cfg, n_total, ms, 27, strays_after_step=ctx.stray_count())
+    if cfg.steps > 1:
+        # configs[1]: one step, then cfg.steps - 1 more with the fields held fixed, state never restored
+        for kind in ("dense", "resident"):
+            restore_sorted()
+            if kind == "resident":
+                for s in range(nsp):
+                    ctx.make_resident(s, 0.5)
+            torch.cuda.synchronize()
+            r0, l0 = ctx.resort_count(), ctx.relayout_count()
+            ms, strays = [], []
+            for _ in range(cfg.steps):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(); step(); e1.record()
+                torch.cuda.synchronize()
+                ms.append(e0.elapsed_time(e1))
+                strays.append(ctx.stray_count())
+            tot = sum(ms)
+            out[name][f"protocol_{kind}"] = {
+                "steps": cfg.steps, "ms_per_step": tot / cfg.steps, "ms_each": [round(v, 3) for v in ms],
+                "particles_per_s": n_total * cfg.steps / (tot * 1e-3),
+                "frac": n_total * cfg.steps / (tot * 1e-3) / config_roofline_pps(cfg, n_total, 27),
+                "strays_per_step": strays, "resorts": ctx.resort_count() - r0, "relayouts": ctx.relayout_count() - l0,
+                **({"slack": 0.5} if kind == "resident" else {})}
+    ctx.close()
+    del work, pristine, M, rho, J, E, B
+    torch.cuda.empty_cache()
+    return out
 
 
 def measure_with_segments(args, cfg, ctx, restore_arrays, one_step, world):
