@@ -48,7 +48,8 @@ enum ecsim_status {
     ECSIM_ERR_WORKSPACE = -3,   /* workspace missing or smaller than ecsim_workspace_bytes() */
     ECSIM_ERR_CUDA = -4,        /* a CUDA call failed; text via ecsim_last_error() */
     ECSIM_ERR_NOMEM = -5,       /* host allocation failed */
-    ECSIM_ERR_OVERFLOW = -6     /* resident species: a push found segments AND the overflow list full; particles were dropped */
+    ECSIM_ERR_OVERFLOW = -6     /* resident species: its last push found segments AND the overflow list full; that push was
+                                   undone, no particle is lost (see ecsim_make_resident) */
 };
 
 /* `accumulate` argument of the push_and_moments calls. */
@@ -170,12 +171,20 @@ int ecsim_push_all(ecsim_ctx *ctx, const double *E_theta, const double *B, doubl
  * cell-major order; also works, as a plain copy, for a species that is not resident).
  * (A species loaded with sorted = 0 is sorted in place first -- its arrays are permuted -- so that the copy is sequential.)
  * ecsim_make_resident synchronises the stream once (it checks the data-dependent slot count against the buffer);
- * slack in [0, 4], typically 0.25.  All species of one *_all call must be of one kind (all resident or none). */
+ * slack in [0, 4], typically 0.25.  All species of one *_all call must be of one kind (all resident or none).
+ * When a push finds a cell's segment AND the overflow list full, no particle is lost: the push writes the idle buffer and
+ * never its input, so the NEXT call that touches the species (any call: they all look at the list's counter first) undoes
+ * that push by swapping the buffers back, lays the pre-push state out afresh, enqueues nothing of its own and returns
+ * ECSIM_ERR_OVERFLOW; ecsim_last_error() names the species.  The moments of a fused call were deposited from the pre-push
+ * state and stay valid: repeat the push of THAT species alone (ecsim_push, same E, B, dt), or make it resident again with
+ * more slack.  ecsim_set_overflow_capacity lowers the list's capacity (1 .. n/8, at least 65536 by default) -- for
+ * tests of this path and for callers that want the error earlier. */
 size_t ecsim_resident_bytes(const ecsim_ctx *ctx, int64_t n_particles, double slack);
 int ecsim_make_resident(ecsim_ctx *ctx, int species, void *dev_buf, size_t bytes, double slack);
 int ecsim_export_particles(ecsim_ctx *ctx, int species, double *x, double *y, double *z, double *u, double *v,
                            double *w, double *q);
 int64_t ecsim_relayout_count(const ecsim_ctx *ctx);
+int ecsim_set_overflow_capacity(ecsim_ctx *ctx, int species, int64_t entries);
 
 /* Reduced dimensionality (L123: "fixPosition ... is only called if the simulation is one or two-dimensional and set the
  * particle position along the same line or on the same plane.  This step is necessary to ensure the correctness of the

@@ -64,6 +64,7 @@ _PROTOS = {
     "ecsim_make_resident": (_c.c_int, [_P, _c.c_int, _P, _c.c_size_t, _c.c_double]),
     "ecsim_export_particles": (_c.c_int, [_P, _c.c_int] + [_P] * 7),
     "ecsim_relayout_count": (_c.c_int64, [_P]),
+    "ecsim_set_overflow_capacity": (_c.c_int, [_P, _c.c_int, _c.c_int64]),
     "ecsim_set_host_pipeline": (_c.c_int, [_P, _c.c_int]),
     "ecsim_host_pipelined_count": (_c.c_int64, [_P]),
     "ecsim_apply_M": (_c.c_int, [_P, _P, _P, _P, _c.c_int]),
@@ -277,6 +278,9 @@ class Ecsim:
 
     def host_pipelined_count(self) -> int:
         return int(self.L.ecsim_host_pipelined_count(self.h))
+
+    def set_overflow_capacity(self, species: int, entries: int):
+        _check(self.L.ecsim_set_overflow_capacity(self.h, species, int(entries)), "ecsim_set_overflow_capacity")
 
     def relayout_count(self) -> int:
         return int(self.L.ecsim_relayout_count(self.h))

@@ -194,7 +194,7 @@ extern "C" const char* ecsim_strerror(int status)
     case ECSIM_ERR_WORKSPACE: return "workspace missing or too small";
     case ECSIM_ERR_CUDA: return "CUDA call failed (see ecsim_last_error)";
     case ECSIM_ERR_NOMEM: return "host allocation failed";
-    case ECSIM_ERR_OVERFLOW: return "resident species: segments and overflow list full, particles were dropped";
+    case ECSIM_ERR_OVERFLOW: return "resident species: segments and overflow list full, the last push of that species was undone (see ecsim_last_error)";
     default: return "unknown status";
     }
 }
@@ -796,9 +796,44 @@ static int resident_settle(ecsim_ctx* c, int s)
     if (!sp.res.on || !sp.leavers_pending) return ECSIM_OK;
     CK(cudaEventSynchronize(sp.leavers_event));
     sp.leavers_pending = false;
-    if (c->h_ovf[s] > sp.res.ovf_cap) return ECSIM_ERR_OVERFLOW;
+    if (c->h_ovf[s] > sp.res.ovf_cap) {
+        // The last push found a cell's segment AND the overflow list full: the particles beyond the list's capacity
+        // were not written anywhere in the buffer it filled.  The buffer it READ -- with its run tables and its own
+        // overflow list -- is untouched (a gapped push never writes its input), so the push is undone by swapping back:
+        // nothing is lost.  A fresh layout of that state gives every cell its slack again, so that the repeated push
+        // has room where this one had none.
+        const uint32_t wanted = c->h_ovf[s];
+        sp.res.cur = 1 - sp.res.cur;
+        sp.res.ovf_cur = 1 - sp.res.ovf_cur;
+        c->h_ovf[s] = 0;
+        const int rrc = resident_relayout(c, s, true);
+        if (rrc) return rrc;
+        snprintf(g_last_error, sizeof(g_last_error),
+                 "resident species %d: its last push needed %u overflow entries, the list holds %u; that push has been "
+                 "undone (no particle lost, the species is at its pre-push state, laid out afresh): repeat ecsim_push for "
+                 "this species, or make it resident again with more slack", s, wanted, sp.res.ovf_cap);
+        return ECSIM_ERR_OVERFLOW;
+    }
     sp.stray_debt += (double)c->h_ovf[s];
     if (c->h_ovf[s] > 0 && sp.stray_debt > 0.25 * c->resort_fraction * (double)sp.n) return resident_relayout(c, s, true);   // (a homeless particle costs ~4x a stray)
+    return ECSIM_OK;
+}
+
+// Lower the capacity of a resident species' overflow list (never above what ecsim_make_resident carved).  The list is
+// [7][capacity]: the capacity is also its stride, so it can only change while the list is empty.
+extern "C" int ecsim_set_overflow_capacity(ecsim_ctx* c, int s, int64_t entries)
+{
+    int rc = check_species(c, s);
+    if (rc) return rc;
+    SpeciesHost& sp = c->sp[s];
+    if (!sp.res.on || entries < 1 || entries > (int64_t)resident_ovf_cap(sp.n)) return ECSIM_ERR_INVALID_ARG;
+    rc = resident_settle(c, s);
+    if (rc) return rc;
+    if (c->h_ovf[s] != 0) {
+        rc = resident_relayout(c, s, true);            // empties the list into fresh segments
+        if (rc) return rc;
+    }
+    sp.res.ovf_cap = (uint32_t)entries;
     return ECSIM_OK;
 }
 

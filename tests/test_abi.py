@@ -72,6 +72,7 @@ def test_null_context_is_an_error_not_a_crash(L):
     assert L.ecsim_apply_M(None, None, None, None, 0) == -1
     assert L.ecsim_set_m_layout(None, 0) == -1
     assert L.ecsim_relayout_count(None) == 0
+    assert L.ecsim_set_overflow_capacity(None, 0, 10) == -1
     assert L.ecsim_validate_particles(None, 0) == -1
     assert L.ecsim_destroy(None) == 0
 

@@ -304,3 +304,48 @@ def test_resident_and_dense_species_cannot_share_a_call():
     ctx.push_and_moments_all(E, B, cfg.dt, cfg.theta, rho, J, M)
     torch.cuda.synchronize()
     ctx.close()
+
+
+def test_resident_overflow_undoes_the_push_and_loses_nobody():
+    """Segments with next to no slack, hot particles and an overflow list of FOUR entries: the push cannot place its
+    leavers.  The next call must report ECSIM_ERR_OVERFLOW with the species back at its pre-push state, bit for bit, and
+    every particle still there; with room in the list again the repeated push then equals the oracle's step, and the
+    moments the fused call deposited (from the pre-push state) were right all along."""
+    base = wl.config(0, (6, 6, 6))
+    hot = tuple(dataclasses.replace(sp, vth=v) for sp, v in zip(base.species, (1.0, 0.5)))
+    cfg = dataclasses.replace(base, dt=0.2, ppc=40, species=hot)
+    E, B = wl.gen_fields(cfg)
+    E_c, B_c = E.cuda(), B.cuda()
+    sp = cfg.species[0]
+    q0 = sp.q_sign * cfg.q_abs
+    p = to_numpy(wl.gen_species(cfg, 0))
+    p["q"] = _tag_ids(p["q"], q0)
+    n = p["x"].shape[0]
+    ctx = make_ctx(cfg, n, n_species=1)
+    ctx.load_particles(0, sp.qom, to_cuda(from_numpy(p)), sorted=False)
+    ctx.make_resident(0, 0.0)
+    ctx.set_overflow_capacity(0, 4)
+    with pytest.raises(pk.EcsimError, match="invalid"):
+        ctx.set_overflow_capacity(0, 0)
+    before = _by_id(_export(ctx, 0, n), q0)
+    for k in PKEYS:
+        assert np.array_equal(before[k], p[k])
+    rho, J, M = alloc_moments(cfg.nodes, 1)
+    ctx.push_and_moments(0, E_c, B_c, cfg.dt, cfg.theta, rho[0], J[0], M)      # enqueued; the overflow is found later
+    torch.cuda.synchronize()
+    with pytest.raises(pk.EcsimError, match="undone"):
+        _export(ctx, 0, n)
+    after = _by_id(_export(ctx, 0, n), q0)                                      # the call after the error works again
+    assert np.array_equal(_ids(after["q"], q0), np.arange(n)), "a particle was lost or duplicated"
+    for k in PKEYS:
+        assert np.array_equal(after[k], before[k]), f"{k}: not the pre-push state"
+    ref = {k: before[k].copy() for k in PKEYS}
+    m = oracle.Moments(cfg.nodes)
+    oracle.step(grid_of(cfg), sp.qom, cfg.dt, ref, E.numpy(), B.numpy(), m)
+    assert_moments_close(rho[0], J[0], M, m, "moments of the call whose push was undone")
+    ctx.set_overflow_capacity(0, 65536)                                         # what make_resident carved
+    ctx.push(0, E_c, B_c, cfg.dt, cfg.theta)
+    got = _by_id(_export(ctx, 0, n), q0)
+    assert np.array_equal(_ids(got["q"], q0), np.arange(n))
+    assert_particles_close(got, ref, cfg, "repeated push")
+    ctx.close()
