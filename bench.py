@@ -642,6 +642,7 @@ def measure_sustained(args, cfg, ctx, restore_arrays, work, E, B, rho, J, M, n_s
             for s in range(nsp):
                 ctx.make_resident(s, 0.5)
         torch.cuda.synchronize()
+        lent = [ctx.resident_bytes(int(work[s]["x"].numel()), 0.5) for s in range(nsp)] if kind != "dense" else None
         r0, l0 = ctx.resort_count(), ctx.relayout_count()
         ms, strays, leavers = [], [], []
         for _ in range(n_steps):
@@ -664,6 +665,9 @@ def measure_sustained(args, cfg, ctx, restore_arrays, work, E, B, rho, J, M, n_s
                      "north_star_frac": n_total * n_steps / (tot * 1e-3) / NORTH_STAR_ROOFLINE_PPS,
                      "strays_per_step": strays, "leavers_per_step": leavers,
                      "resorts": ctx.resort_count() - r0, "relayouts": ctx.relayout_count() - l0}
+        if lent is not None:
+            out[kind]["slack"] = 0.5
+            out[kind]["lent_bytes_per_species"] = lent      # the gapped double buffers + tables the caller lends (ecsim_resident_bytes)
     return out
 
 
